@@ -1,0 +1,140 @@
+/* apex4.h -- C ABI of the B200-native APEX4 W4A4 hot path (arxiv/paper_2606_08761).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines):
+ *   Eq. 7  symmetric INT4 group quantizer
+ *        S = fp16(absmax / 7),  q = clamp(rne(x / S), -8, 7),  scales kept in FP16
+ *   Eq. 8  group-dequantised GEMM
+ *        Y[m,n] = sum_g sA[m,g] * sW[n,g] * (sum_{k in g} qA[m,k] * qW[n,k])
+ *        exact INT32 partial sums per K-group on the tensor cores (tcgen05.mma kind::i8,
+ *        operands widened INT4->INT8 in shared memory because sm_100a has no 4-bit integer
+ *        MMA kind), INT32->FP32 + scale multiply on the CUDA cores, FP32 accumulation.
+ *   3.2.2  granularity: uniform g, per-channel (g = K), mixed policy.
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless its comment says HOST.  The caller allocates and owns
+ *     every buffer; the library never allocates, frees or keeps a pointer after the call returns.
+ *   - Every call only enqueues work on `stream` (a cudaStream_t passed as void*, NULL = default
+ *     stream) and never synchronises (except apex4_measure_rho and the *_host helpers, which say so).
+ *   - Return value: an apex4_status.  Arguments are validated before anything is launched; a failed
+ *     launch returns APEX4_ERR_CUDA.  Nothing is printed, nothing aborts.
+ *   - Shapes: X[M,K], W[N,K], Y[M,N] dense row-major (last index contiguous).  K % 128 == 0,
+ *     N % 8 == 0, M >= 1.  Group size g: 32, 64, or a multiple of 128 that divides K (128, 256, 512,
+ *     1024, ..., K).  Pointers 16-byte aligned.
+ *   - Device layouts (opaque to the caller; sizes from the *_bytes queries below):
+ *       packed codes  "PT4": rows padded to Rp = roundup(R,128); blob (rt, kb) of 128 rows x 128 k
+ *                     = 8192 contiguous bytes at ((rt * K/128 + kb) * 8192); inside a blob row r
+ *                     occupies 64 bytes and its 16-byte chunks / nibbles are permuted so that the
+ *                     in-kernel widening lands directly in the 128B-swizzled UMMA operand layout
+ *                     (see csrc/apex4_layout.cuh).  apex4_unpack_codes inverts it.
+ *       scales        "ST16": FP16, tile-major [Rp/128][G][128], G = K/g: element (r, gamma) at
+ *                     ((r/128) * G + gamma) * 128 + r % 128.  apex4_scales_to_natural inverts it.
+ */
+#ifndef APEX4_H_
+#define APEX4_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  APEX4_OK = 0,
+  APEX4_ERR_INVALID_ARG = 1,       /* null pointer, non-positive size, unknown enum */
+  APEX4_ERR_UNSUPPORTED_SHAPE = 2, /* K % 128, N % 8, group size not supported / not dividing K */
+  APEX4_ERR_ALIGNMENT = 3,         /* a pointer is not 16-byte aligned */
+  APEX4_ERR_WORKSPACE = 4,         /* workspace NULL or smaller than apex4_workspace_bytes() */
+  APEX4_ERR_CUDA = 5,              /* a CUDA runtime call / kernel launch failed */
+  APEX4_ERR_ARCH = 6               /* device is not compute capability 10.0 (sm_100a) */
+} apex4_status;
+
+/* granularity mode: how group_size is resolved */
+typedef enum {
+  APEX4_GRAN_GROUP = 0,      /* g = group_size */
+  APEX4_GRAN_CHANNEL = 1,    /* g = K (one scale per token row / per output channel), group_size ignored */
+  APEX4_GRAN_MIXED = 2,      /* paper's mix: down_proj, v_proj -> 32; every other layer -> K */
+  APEX4_GRAN_MIXED_G128 = 3  /* BASELINE.json wording: the fine layers at 128, others per-channel */
+} apex4_gran;
+
+typedef enum {
+  APEX4_LAYER_OTHER = 0, APEX4_LAYER_Q = 1, APEX4_LAYER_K = 2, APEX4_LAYER_V = 3, APEX4_LAYER_QKV = 4,
+  APEX4_LAYER_O = 5, APEX4_LAYER_GATE = 6, APEX4_LAYER_UP = 7, APEX4_LAYER_GATE_UP = 8,
+  APEX4_LAYER_DOWN = 9
+} apex4_layer;
+
+typedef enum { APEX4_OUT_F16 = 0, APEX4_OUT_F32 = 1 } apex4_out;
+
+/* ---- host-side queries (no CUDA work) ------------------------------------------------------- */
+
+/* Group size a call with these arguments runs at, or a negative apex4_status on invalid input.
+ * PAPER.md:162-166, 183.  Pure host function. */
+int apex4_resolve_group_size(int K, int group_size, int gran, int layer);
+
+/* Bytes of the PT4 packed-code buffer for an operand with R rows (M for activations, N for weights). */
+size_t apex4_packed_bytes(int R, int K);
+/* Number of FP16 elements of the ST16 scale buffer for R rows at resolved group size g. */
+size_t apex4_scale_elems(int R, int K, int g);
+/* Bytes of workspace apex4_w4a4_gemm needs for this problem (0 if none).  The workspace must be
+ * zero-filled once by the caller before its first use; every call leaves it zero-filled again. */
+size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer);
+
+const char* apex4_status_string(int status);
+
+/* ---- a1: online activation quantizer (Eq. 7) -------------------------- */
+/* x_f16 [M,K] FP16 -> qA_packed (PT4, apex4_packed_bytes(M,K)) + sA_f16 (ST16, apex4_scale_elems). */
+int apex4_quantize_act(const void* x_f16, int M, int K, int group_size, int gran, int layer,
+                       void* qA_packed, void* sA_f16, void* stream);
+
+/* ---- a0: offline weight quantize + pack (Eq. 7) --------------------------- */
+/* w_f16 [N,K] FP16 -> qW_packed (PT4) + sW_f16 (ST16). Same arithmetic as the activation quantizer. */
+int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran, int layer,
+                       void* qW_packed, void* sW_f16, void* stream);
+/* Offline-calibrated path (Alg. 1 output): codes [R,K] int8 in [-8,7] (row-major)
+ * -> PT4.  Values outside [-8,7] are taken modulo 16 (low nibble). */
+int apex4_pack_codes(const int8_t* codes, int R, int K, void* q_packed, void* stream);
+/* natural FP16 scales [R,G] row-major -> ST16 (padding rows zero-filled), and back. */
+int apex4_scales_from_natural(const void* s_nat_f16, int R, int G, void* s_tiled_f16, void* stream);
+int apex4_scales_to_natural(const void* s_tiled_f16, int R, int G, void* s_nat_f16, void* stream);
+/* PT4 -> codes [R,K] int8 (verification twin of the packers; works for activations and weights). */
+int apex4_unpack_codes(const void* q_packed, int R, int K, int8_t* codes, void* stream);
+
+/* ---- a2..a7: the W4A4 group-dequant GEMM (Eq. 8) ----------------------------- */
+/* Y [M,N] (FP16 or FP32 per out_dtype) = sum_g sA sW P_g.  qA/sA from apex4_quantize_act, qW/sW
+ * from apex4_pack_weights, both at the same resolved group size (G_a = G_w).
+ * workspace: apex4_workspace_bytes() bytes (may be NULL when that is 0). */
+int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
+                    const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
+                    int gran, int layer, void* workspace, size_t workspace_bytes, void* stream);
+
+/* End-to-end convenience over the three calls above with HOST activations and HOST output:
+ * x_host_f16 [M,K] (HOST, pinned for true asynchrony) -> cudaMemcpyAsync -> apex4_quantize_act ->
+ * apex4_w4a4_gemm (weights qW/sW pre-packed on the DEVICE) -> cudaMemcpyAsync -> y_host [M,N] (HOST).
+ * scratch: DEVICE memory of apex4_linear_host_scratch_bytes() bytes, zero-filled once by the caller
+ * (its head is the GEMM workspace) and reusable across calls of the same shape.  Enqueues only. */
+size_t apex4_linear_host_scratch_bytes(int M, int N, int K, int group_size, int gran, int layer);
+int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const void* sW_f16,
+                           void* y_host, int M, int N, int K, int group_size, int gran, int layer,
+                           int out_dtype, void* scratch, size_t scratch_bytes, void* stream);
+
+/* Verification export: the exact per-group INT32 sums P[m,n,gamma] the tensor cores produced, for the
+ * window m in [m0,m1), n in [n0,n1): P_out [(m1-m0), (n1-n0), G] int32 row-major.  Runs the same
+ * tcgen05 kernel as apex4_w4a4_gemm (same tiles, same pipeline) with the TMEM accumulators dumped
+ * by the epilogue. */
+int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, int N, int K,
+                           int group_size, int gran, int layer, int m0, int m1, int n0, int n1,
+                           int32_t* P_out, void* stream);
+
+/* ---- rho microbenchmark (Eq. 1-2; Table 1) -------------------- */
+/* Measures on the current device: dense INT8 tcgen05.mma rate (TOPS), FP32 FMA rate (TFLOPS),
+ * INT32->FP32 conversion rate (Gop/s) and rho = int8_tops / fp32_tflops.  out[] is a HOST array of
+ * at least 8 doubles: {int8_tops, fp32_tflops, i2f_gops, rho, tmem_ld_gbs, sm_clock_mhz, int8_mac_per_clk_per_sm,
+ * tmem_ld_bytes_per_clk_per_sm}.
+ * Synchronises the stream; allocates and frees its own small device scratch (the only call that
+ * does). */
+int apex4_measure_rho(double* out_host, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* APEX4_H_ */

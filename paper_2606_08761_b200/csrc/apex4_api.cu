@@ -1,0 +1,339 @@
+// apex4_api.cu -- the C ABI of include/apex4.h: argument validation, granularity policy (a8),
+// dispatch between the normal and the swapped/split-K orientation of the GEMM kernel.
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+
+#include "../../include/apex4.h"
+#include "apex4_gemm.cuh"
+#include "apex4_layout.cuh"
+
+namespace apex4 {
+cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, cudaStream_t st);
+bool quantize_supports_group(int g);
+cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, cudaStream_t st);
+cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, cudaStream_t st);
+cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st);
+cudaError_t launch_scales_to_natural(const void* tiled, int R, int G, void* nat, cudaStream_t st);
+int measure_rho(double* out, cudaStream_t st);
+}  // namespace apex4
+
+using namespace apex4;
+
+namespace {
+
+constexpr int kCounterInts = 4096;   // split-K arrival counters live at the front of the workspace
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int check_arch() {
+  static int cached = -1;
+  if (cached >= 0) return cached;
+  int dev = 0, major = 0, minor = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return APEX4_ERR_CUDA;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess)
+    return APEX4_ERR_CUDA;
+  cached = (major == 10 && minor == 0) ? APEX4_OK : APEX4_ERR_ARCH;
+  return cached;
+}
+
+// a8: group size from (K, group_size, gran, layer).  PAPER.md:162-166, 183; reading R11.
+int resolve_g(int K, int group_size, int gran, int layer) {
+  if (K <= 0 || K % kBlockK != 0) return -APEX4_ERR_UNSUPPORTED_SHAPE;
+  if (layer < APEX4_LAYER_OTHER || layer > APEX4_LAYER_DOWN) return -APEX4_ERR_INVALID_ARG;
+  int g;
+  switch (gran) {
+    case APEX4_GRAN_GROUP: g = group_size; break;
+    case APEX4_GRAN_CHANNEL: g = K; break;
+    case APEX4_GRAN_MIXED:
+      g = (layer == APEX4_LAYER_V || layer == APEX4_LAYER_DOWN) ? 32 : K;
+      break;
+    case APEX4_GRAN_MIXED_G128:
+      g = (layer == APEX4_LAYER_V || layer == APEX4_LAYER_DOWN) ? 128 : K;
+      break;
+    default: return -APEX4_ERR_INVALID_ARG;
+  }
+  if (g <= 0) return -APEX4_ERR_INVALID_ARG;
+  const bool ok = (g == 32 || g == 64 || (g % kBlockK == 0)) && (K % g == 0);
+  if (!ok) return -APEX4_ERR_UNSUPPORTED_SHAPE;
+  if (!quantize_supports_group(g)) return -APEX4_ERR_UNSUPPORTED_SHAPE;
+  return g;
+}
+
+struct Dispatch {
+  int swap, nc, splits, kb_per_split;
+};
+
+// test hook (apex4_debug_set_dispatch): -1 = automatic
+int g_force_swap = -1, g_force_nc = -1, g_force_splits = -1;
+
+Dispatch choose_dispatch(int M, int N, int K, int g) {
+  Dispatch d;
+  const int KB = K / kBlockK;
+  const int kbpg = g > kBlockK ? g / kBlockK : 1;
+  const int units = KB / kbpg;   // indivisible k units (whole groups)
+  d.swap = (g_force_swap >= 0) ? g_force_swap : (M <= 64 ? 1 : 0);
+  const int Rn = d.swap ? N : M, Cn = d.swap ? M : N;
+  if (g_force_nc > 0) d.nc = g_force_nc;
+  else if (Cn <= 16) d.nc = 16;
+  else if (Cn <= 32) d.nc = 32;
+  else if (Cn <= 64) d.nc = 64;
+  else if (Cn <= 128) d.nc = 128;
+  else d.nc = 256;
+  const int r_tiles = (Rn + kTileRows - 1) / kTileRows;
+  int c_tiles = (Cn + d.nc - 1) / d.nc;
+  if (g_force_nc <= 0 && d.nc == 256 && r_tiles * c_tiles < 148 && Cn > 128) {
+    d.nc = 128;   // more, smaller tiles when the grid would not fill the chip
+    c_tiles = (Cn + 127) / 128;
+  }
+  const int tiles = r_tiles * c_tiles;
+  int splits = 1;
+  if (g_force_splits > 0) splits = g_force_splits;
+  else if (tiles < 148) {
+    const int slots = d.nc <= 64 ? 296 : 148;   // small-NC kernels fit two CTAs per SM
+    splits = slots / tiles;
+  }
+  if (splits > units) splits = units;
+  if (splits < 1) splits = 1;
+  const int units_per = (units + splits - 1) / splits;
+  d.kb_per_split = units_per * kbpg;
+  d.splits = (units + units_per - 1) / units_per;
+  return d;
+}
+
+int validate_gemm_shape(int M, int N, int K) {
+  if (M < 1 || N < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
+  if (K % kBlockK != 0 || N % 8 != 0 || K > 32768) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  return APEX4_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* apex4_status_string(int status) {
+  switch (status) {
+    case APEX4_OK: return "ok";
+    case APEX4_ERR_INVALID_ARG: return "invalid argument";
+    case APEX4_ERR_UNSUPPORTED_SHAPE: return "unsupported shape or group size";
+    case APEX4_ERR_ALIGNMENT: return "pointer not 16-byte aligned";
+    case APEX4_ERR_WORKSPACE: return "workspace missing or too small";
+    case APEX4_ERR_CUDA: return "CUDA error";
+    case APEX4_ERR_ARCH: return "device is not sm_100a (compute capability 10.0)";
+    default: return "unknown status";
+  }
+}
+
+int apex4_resolve_group_size(int K, int group_size, int gran, int layer) {
+  return resolve_g(K, group_size, gran, layer);
+}
+
+size_t apex4_packed_bytes(int R, int K) {
+  if (R < 1 || K < 1 || K % kBlockK != 0) return 0;
+  return pt4_bytes(R, K);
+}
+size_t apex4_scale_elems(int R, int K, int g) {
+  if (R < 1 || K < 1 || g < 1 || K % g != 0) return 0;
+  return st16_elems(R, K / g);
+}
+
+size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer) {
+  if (validate_gemm_shape(M, N, K) != APEX4_OK) return 0;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return 0;
+  const Dispatch d = choose_dispatch(M, N, K, g);
+  if (d.splits <= 1) return 0;
+  return static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4;
+}
+
+static int quantize_common(const void* x, int R, int K, int group_size, int gran, int layer, void* q,
+                           void* s, void* stream) {
+  if (!x || !q || !s || R < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
+  if (K > 32768) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  if (!aligned16(x) || !aligned16(q) || !aligned16(s)) return APEX4_ERR_ALIGNMENT;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_quantize(x, R, K, g, q, s, static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
+}
+
+int apex4_quantize_act(const void* x_f16, int M, int K, int group_size, int gran, int layer,
+                       void* qA_packed, void* sA_f16, void* stream) {
+  return quantize_common(x_f16, M, K, group_size, gran, layer, qA_packed, sA_f16, stream);
+}
+int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran, int layer,
+                       void* qW_packed, void* sW_f16, void* stream) {
+  return quantize_common(w_f16, N, K, group_size, gran, layer, qW_packed, sW_f16, stream);
+}
+
+int apex4_pack_codes(const int8_t* codes, int R, int K, void* q_packed, void* stream) {
+  if (!codes || !q_packed || R < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
+  if (K % kBlockK != 0) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(codes) || !aligned16(q_packed)) return APEX4_ERR_ALIGNMENT;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_pack_codes(codes, R, K, q_packed, static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
+}
+int apex4_unpack_codes(const void* q_packed, int R, int K, int8_t* codes, void* stream) {
+  if (!codes || !q_packed || R < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
+  if (K % kBlockK != 0) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(codes) || !aligned16(q_packed)) return APEX4_ERR_ALIGNMENT;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_unpack_codes(q_packed, R, K, codes, static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
+}
+int apex4_scales_from_natural(const void* s_nat, int R, int G, void* s_tiled, void* stream) {
+  if (!s_nat || !s_tiled || R < 1 || G < 1) return APEX4_ERR_INVALID_ARG;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_scales_from_natural(s_nat, R, G, s_tiled, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
+}
+int apex4_scales_to_natural(const void* s_tiled, int R, int G, void* s_nat, void* stream) {
+  if (!s_nat || !s_tiled || R < 1 || G < 1) return APEX4_ERR_INVALID_ARG;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_scales_to_natural(s_tiled, R, G, s_nat, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
+}
+
+static void fill_params(GemmParams& p, const Dispatch& d, const void* qA, const void* sA,
+                        const void* qW, const void* sW, int M, int N, int K, int g) {
+  memset(&p, 0, sizeof(p));
+  if (d.swap) {
+    p.qR = static_cast<const uint8_t*>(qW); p.sR = static_cast<const __half*>(sW); p.R = N;
+    p.qC = static_cast<const uint8_t*>(qA); p.sC = static_cast<const __half*>(sA); p.C = M;
+  } else {
+    p.qR = static_cast<const uint8_t*>(qA); p.sR = static_cast<const __half*>(sA); p.R = M;
+    p.qC = static_cast<const uint8_t*>(qW); p.sC = static_cast<const __half*>(sW); p.C = N;
+  }
+  p.K = K; p.g = g; p.G = K / g; p.ldY = N; p.swap = d.swap;
+  p.splits = d.splits; p.kb_per_split = d.kb_per_split;
+}
+
+int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
+                    const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
+                    int gran, int layer, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!qA_packed || !sA_f16 || !qW_packed || !sW_f16 || !Y) return APEX4_ERR_INVALID_ARG;
+  if (out_dtype != APEX4_OUT_F16 && out_dtype != APEX4_OUT_F32) return APEX4_ERR_INVALID_ARG;
+  int v = validate_gemm_shape(M, N, K);
+  if (v != APEX4_OK) return v;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  if (!aligned16(qA_packed) || !aligned16(sA_f16) || !aligned16(qW_packed) || !aligned16(sW_f16) ||
+      !aligned16(Y))
+    return APEX4_ERR_ALIGNMENT;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  const Dispatch d = choose_dispatch(M, N, K, g);
+  GemmParams p;
+  fill_params(p, d, qA_packed, sA_f16, qW_packed, sW_f16, M, N, K, g);
+  p.Y = Y; p.out_f32 = (out_dtype == APEX4_OUT_F32);
+  if (d.splits > 1) {
+    const size_t need = static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4;
+    const int Rn = d.swap ? N : M, Cn = d.swap ? M : N;
+    const long long tiles = static_cast<long long>((Rn + kTileRows - 1) / kTileRows) * ((Cn + d.nc - 1) / d.nc);
+    if (!workspace || workspace_bytes < need || !aligned16(workspace)) return APEX4_ERR_WORKSPACE;
+    if (tiles > kCounterInts) return APEX4_ERR_UNSUPPORTED_SHAPE;
+    p.counters = static_cast<int*>(workspace);
+    p.ws = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + kCounterInts * 4);
+  }
+  return launch_gemm(p, d.nc, false, static_cast<cudaStream_t>(stream)) == cudaSuccess ? APEX4_OK
+                                                                                       : APEX4_ERR_CUDA;
+}
+
+int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, int N, int K,
+                           int group_size, int gran, int layer, int m0, int m1, int n0, int n1,
+                           int32_t* P_out, void* stream) {
+  if (!qA_packed || !qW_packed || !P_out) return APEX4_ERR_INVALID_ARG;
+  int v = validate_gemm_shape(M, N, K);
+  if (v != APEX4_OK) return v;
+  if (m0 < 0 || m1 > M || m0 >= m1 || n0 < 0 || n1 > N || n0 >= n1) return APEX4_ERR_INVALID_ARG;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  const Dispatch d = choose_dispatch(M, N, K, g);
+  GemmParams p;
+  // scales are not needed for the integer sums; any valid ST16-sized device memory would do, the
+  // packed code buffers are large enough and are only read
+  fill_params(p, d, qA_packed, qA_packed, qW_packed, qW_packed, M, N, K, g);
+  p.Y = nullptr; p.P_out = P_out; p.pm0 = m0; p.pm1 = m1; p.pn0 = n0; p.pn1 = n1;
+  return launch_gemm(p, d.nc, true, static_cast<cudaStream_t>(stream)) == cudaSuccess ? APEX4_OK
+                                                                                      : APEX4_ERR_CUDA;
+}
+
+static size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+
+size_t apex4_linear_host_scratch_bytes(int M, int N, int K, int group_size, int gran, int layer) {
+  if (validate_gemm_shape(M, N, K) != APEX4_OK) return 0;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return 0;
+  return align256(static_cast<size_t>(M) * K * 2) + align256(pt4_bytes(M, K)) +
+         align256(st16_elems(M, K / g) * 2) + align256(static_cast<size_t>(M) * N * 4) +
+         align256(static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4);
+}
+
+int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const void* sW_f16,
+                           void* y_host, int M, int N, int K, int group_size, int gran, int layer,
+                           int out_dtype, void* scratch, size_t scratch_bytes, void* stream) {
+  if (!x_host_f16 || !qW_packed || !sW_f16 || !y_host || !scratch) return APEX4_ERR_INVALID_ARG;
+  int v = validate_gemm_shape(M, N, K);
+  if (v != APEX4_OK) return v;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  if (scratch_bytes < apex4_linear_host_scratch_bytes(M, N, K, group_size, gran, layer) ||
+      !aligned16(scratch))
+    return APEX4_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  uint8_t* base = static_cast<uint8_t*>(scratch);
+  uint8_t* ws = base;   // the split-K workspace comes first so that it stays zero-filled across calls
+  const size_t ws_bytes = align256(static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4);
+  uint8_t* xd = ws + ws_bytes;
+  uint8_t* qa = xd + align256(static_cast<size_t>(M) * K * 2);
+  uint8_t* sa = qa + align256(pt4_bytes(M, K));
+  uint8_t* yd = sa + align256(st16_elems(M, K / g) * 2);
+  const size_t ybytes = static_cast<size_t>(M) * N * (out_dtype == APEX4_OUT_F32 ? 4 : 2);
+  if (cudaMemcpyAsync(xd, x_host_f16, static_cast<size_t>(M) * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return APEX4_ERR_CUDA;
+  int rc = apex4_quantize_act(xd, M, K, group_size, gran, layer, qa, sa, stream);
+  if (rc != APEX4_OK) return rc;
+  rc = apex4_w4a4_gemm(qa, sa, qW_packed, sW_f16, yd, out_dtype, M, N, K, group_size, gran, layer, ws,
+                       ws_bytes, stream);
+  if (rc != APEX4_OK) return rc;
+  if (cudaMemcpyAsync(y_host, yd, ybytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return APEX4_ERR_CUDA;
+  return APEX4_OK;
+}
+
+// test hook, not part of the documented ABI: force orientation / tile width / split factor
+// (-1 = automatic).  Process-global; tests restore it.
+int apex4_debug_set_dispatch(int swap, int nc, int splits) {
+  g_force_swap = swap; g_force_nc = nc; g_force_splits = splits;
+  return APEX4_OK;
+}
+int apex4_debug_get_dispatch(int M, int N, int K, int g, int* out4) {
+  const Dispatch d = choose_dispatch(M, N, K, g);
+  out4[0] = d.swap; out4[1] = d.nc; out4[2] = d.splits; out4[3] = d.kb_per_split;
+  return APEX4_OK;
+}
+
+int apex4_measure_rho(double* out_host, void* stream) {
+  if (!out_host) return APEX4_ERR_INVALID_ARG;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return measure_rho(out_host, static_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"

@@ -1,0 +1,297 @@
+// apex4_quant.cu -- a0/a1 of the hot path: the symmetric INT4 group quantizer of Eq. 7
+// (PAPER.md:146-150), used online for activations and offline for weights, writing the PT4 / ST16
+// device layouts of apex4_layout.cuh; plus the code packer / unpacker and scale re-layout twins.
+//
+// Arithmetic (readings R1-R5 of DESIGN.md): a = max|x| exact in FP16; S = fp16_rn(float(a) / 7.0f)
+// with an IEEE binary32 division; q = clamp(rne(x / float(S)), -8, 7) with an IEEE binary32 division
+// (rne of the binary32 quotient equals rne of the true quotient for FP16 x and S, lemma L1);
+// S == 0 -> q = 0.  Never build this file with -use_fast_math.
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "apex4_layout.cuh"
+
+namespace apex4 {
+
+__device__ __forceinline__ uint32_t hmax2_abs(uint32_t acc, uint32_t v) {
+  __half2 a = *reinterpret_cast<__half2*>(&acc);
+  __half2 b = __habs2(*reinterpret_cast<__half2*>(&v));
+  __half2 m = __hmax2(a, b);
+  return *reinterpret_cast<uint32_t*>(&m);
+}
+
+__device__ __forceinline__ int quant_one(float x, float s) {
+  // s > 0 here.  IEEE division, round-half-to-even, clamp (Eq. 7).
+  int q = __float2int_rn(__fdiv_rn(x, s));
+  return max(-8, min(7, q));
+}
+
+// 32 FP16 values (4 x uint4) -> 16 packed bytes (one PT4 chunk) for blob row rr.
+__device__ __forceinline__ uint4 quant_pack_chunk(const uint4 (&v)[4], float s, int rr) {
+  int code[32];
+  const uint32_t* w = reinterpret_cast<const uint32_t*>(v);
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    __half2 h = *reinterpret_cast<const __half2*>(&w[i]);
+    float2 f = __half22float2(h);
+    code[2 * i] = (s == 0.f) ? 0 : quant_one(f.x, s);
+    code[2 * i + 1] = (s == 0.f) ? 0 : quant_one(f.y, s);
+  }
+  const int swap = rr & 1;   // which 16-element half lands in the low nibbles (apex4_layout.cuh)
+  uint32_t out[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    uint32_t word = 0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int y = 4 * i + b;
+      const int lo = swap ? code[16 + y] : code[y];
+      const int hi = swap ? code[y] : code[16 + y];
+      word |= static_cast<uint32_t>((lo & 0xF) | ((hi & 0xF) << 4)) << (8 * b);
+    }
+    out[i] = word;
+  }
+  return make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+__device__ __forceinline__ float scale_from_absmax_bits(uint32_t amax_bits, __half* S_out) {
+  __half a = __ushort_as_half(static_cast<unsigned short>(amax_bits));
+  float s32 = __fdiv_rn(__half2float(a), 7.0f);
+  __half S = __float2half_rn(s32);
+  *S_out = S;
+  return __half2float(S);
+}
+
+__device__ __forceinline__ size_t chunk_dst_offset(int r, int c, int K) {
+  const int rt = r / kTileRows, rr = r % kTileRows;
+  const int kb = c >> 2, s = c & 3;
+  const int j = s ^ ((rr >> 1) & 3);
+  return pt4_blob_offset(rt, kb, K) + static_cast<size_t>(rr) * kRowBytes + j * 16;
+}
+
+// One thread = one 32-element chunk; a group is GL = g/32 consecutive lanes of a warp (GL in 1..32).
+template <int GL>
+__global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __restrict__ X, int R,
+                                                               int K, uint8_t* __restrict__ q,
+                                                               __half* __restrict__ S) {
+  const int cpr = K / 32;
+  const long long total = static_cast<long long>(R) * cpr;
+  long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const bool active = gid < total;
+  if (!active) gid = total - 1;   // keep the warp converged for the shuffles; results discarded
+  const int r = static_cast<int>(gid / cpr);
+  const int c = static_cast<int>(gid % cpr);
+  const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + c * 32);
+  uint4 v[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) v[i] = __ldg(src + i);
+  uint32_t m = 0;
+  const uint32_t* w = reinterpret_cast<const uint32_t*>(v);
+#pragma unroll
+  for (int i = 0; i < 16; ++i) m = hmax2_abs(m, w[i]);
+  {  // fold the two halves, then across the group's lanes
+    __half2 mm = *reinterpret_cast<__half2*>(&m);
+    __half h = __hmax(__low2half(mm), __high2half(mm));
+    m = __half_as_ushort(h);
+  }
+#pragma unroll
+  for (int d = 1; d < GL; d <<= 1) {
+    uint32_t o = __shfl_xor_sync(0xffffffffu, m, d);
+    __half a = __ushort_as_half(static_cast<unsigned short>(m));
+    __half b = __ushort_as_half(static_cast<unsigned short>(o));
+    m = __half_as_ushort(__hmax(a, b));
+  }
+  __half Sh;
+  const float s = scale_from_absmax_bits(m, &Sh);
+  const uint4 packed = quant_pack_chunk(v, s, r % kTileRows);
+  if (active) {
+    *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c, K)) = packed;
+    if ((c % GL) == 0) S[st16_index(r, c / GL, cpr / GL)] = Sh;
+  }
+}
+
+// One block = one (row, group) with g/32 <= 4 * blockDim chunks; data stays in registers between
+// the absmax pass and the quantize pass.
+constexpr int kLargeThreads = 256;
+constexpr int kLargeUnroll = 4;
+__global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
+    const __half* __restrict__ X, int R, int K, int g, uint8_t* __restrict__ q,
+    __half* __restrict__ S) {
+  const int G = K / g;
+  const int r = blockIdx.x / G;
+  const int gamma = blockIdx.x % G;
+  const int cpg = g / 32;
+  const int c0 = gamma * cpg;
+  __shared__ uint32_t red[kLargeThreads / 32];
+  uint4 v[kLargeUnroll][4];
+  uint32_t m = 0;
+#pragma unroll
+  for (int u = 0; u < kLargeUnroll; ++u) {
+    const int cl = threadIdx.x + u * kLargeThreads;
+    if (cl < cpg) {
+      const uint4* src =
+          reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + (c0 + cl) * 32);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) v[u][i] = __ldg(src + i);
+      const uint32_t* w = reinterpret_cast<const uint32_t*>(v[u]);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) m = hmax2_abs(m, w[i]);
+    }
+  }
+  {
+    __half2 mm = *reinterpret_cast<__half2*>(&m);
+    m = __half_as_ushort(__hmax(__low2half(mm), __high2half(mm)));
+  }
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    uint32_t o = __shfl_xor_sync(0xffffffffu, m, d);
+    m = __half_as_ushort(__hmax(__ushort_as_half(static_cast<unsigned short>(m)),
+                                __ushort_as_half(static_cast<unsigned short>(o))));
+  }
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  m = red[0];
+#pragma unroll
+  for (int i = 1; i < kLargeThreads / 32; ++i)
+    m = __half_as_ushort(__hmax(__ushort_as_half(static_cast<unsigned short>(m)),
+                                __ushort_as_half(static_cast<unsigned short>(red[i]))));
+  __half Sh;
+  const float s = scale_from_absmax_bits(m, &Sh);
+  if (threadIdx.x == 0) S[st16_index(r, gamma, G)] = Sh;
+#pragma unroll
+  for (int u = 0; u < kLargeUnroll; ++u) {
+    const int cl = threadIdx.x + u * kLargeThreads;
+    if (cl < cpg) {
+      const uint4 packed = quant_pack_chunk(v[u], s, r % kTileRows);
+      *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c0 + cl, K)) = packed;
+    }
+  }
+}
+
+// codes int8 [R,K] -> PT4
+__global__ void __launch_bounds__(256) pack_codes_kernel(const int8_t* __restrict__ codes, int R,
+                                                         int K, uint8_t* __restrict__ q) {
+  const int cpr = K / 32;
+  const long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (gid >= static_cast<long long>(R) * cpr) return;
+  const int r = static_cast<int>(gid / cpr), c = static_cast<int>(gid % cpr);
+  const uint4* src = reinterpret_cast<const uint4*>(codes + static_cast<size_t>(r) * K + c * 32);
+  uint4 in[2] = {__ldg(src), __ldg(src + 1)};
+  const int8_t* cd = reinterpret_cast<const int8_t*>(in);
+  const int swap = r & 1;
+  uint32_t out[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    uint32_t word = 0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int y = 4 * i + b;
+      const int lo = swap ? cd[16 + y] : cd[y];
+      const int hi = swap ? cd[y] : cd[16 + y];
+      word |= static_cast<uint32_t>((lo & 0xF) | ((hi & 0xF) << 4)) << (8 * b);
+    }
+    out[i] = word;
+  }
+  *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c, K)) = make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+// PT4 -> codes int8 [R,K]
+__global__ void __launch_bounds__(256) unpack_codes_kernel(const uint8_t* __restrict__ q, int R,
+                                                           int K, int8_t* __restrict__ codes) {
+  const int cpr = K / 32;
+  const long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (gid >= static_cast<long long>(R) * cpr) return;
+  const int r = static_cast<int>(gid / cpr), c = static_cast<int>(gid % cpr);
+  const uint4 p = __ldg(reinterpret_cast<const uint4*>(q + chunk_dst_offset(r, c, K)));
+  const uint8_t* pb = reinterpret_cast<const uint8_t*>(&p);
+  const int swap = r & 1;
+  int8_t out[32];
+#pragma unroll
+  for (int y = 0; y < 16; ++y) {
+    int lo = pb[y] & 0xF, hi = pb[y] >> 4;
+    lo = lo >= 8 ? lo - 16 : lo;
+    hi = hi >= 8 ? hi - 16 : hi;
+    out[y] = static_cast<int8_t>(swap ? hi : lo);
+    out[16 + y] = static_cast<int8_t>(swap ? lo : hi);
+  }
+  uint4* dst = reinterpret_cast<uint4*>(codes + static_cast<size_t>(r) * K + c * 32);
+  dst[0] = *reinterpret_cast<uint4*>(&out[0]);
+  dst[1] = *reinterpret_cast<uint4*>(&out[16]);
+}
+
+__global__ void scales_from_natural_kernel(const __half* __restrict__ nat, int R, int G,
+                                           __half* __restrict__ tiled) {
+  const long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const long long total = static_cast<long long>(round_up(R, kTileRows)) * G;
+  if (gid >= total) return;
+  // gid indexes the tiled buffer: ((rt*G + gamma)*128 + rr)
+  const int rr = static_cast<int>(gid % kTileRows);
+  const long long t = gid / kTileRows;
+  const int gamma = static_cast<int>(t % G);
+  const int r = static_cast<int>(t / G) * kTileRows + rr;
+  tiled[gid] = (r < R) ? nat[static_cast<size_t>(r) * G + gamma] : __float2half_rn(0.f);
+}
+__global__ void scales_to_natural_kernel(const __half* __restrict__ tiled, int R, int G,
+                                         __half* __restrict__ nat) {
+  const long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (gid >= static_cast<long long>(R) * G) return;
+  const int r = static_cast<int>(gid / G), gamma = static_cast<int>(gid % G);
+  nat[gid] = tiled[st16_index(r, gamma, G)];
+}
+
+// ---------------------------------------------------------------------------------- launchers
+cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, cudaStream_t st) {
+  const __half* X = static_cast<const __half*>(x);
+  uint8_t* Q = static_cast<uint8_t*>(q);
+  __half* S = static_cast<__half*>(s);
+  const int gl = g / 32;
+  const long long total = static_cast<long long>(R) * (K / 32);
+  const unsigned blocks = static_cast<unsigned>((total + 255) / 256);
+  const bool pow2 = (gl & (gl - 1)) == 0;
+  if (pow2 && gl <= 32) {
+    switch (gl) {
+      case 1: quantize_small_g_kernel<1><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+      case 2: quantize_small_g_kernel<2><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+      case 4: quantize_small_g_kernel<4><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+      case 8: quantize_small_g_kernel<8><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+      case 16: quantize_small_g_kernel<16><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+      default: quantize_small_g_kernel<32><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+    }
+  } else {
+    if (gl > kLargeThreads * kLargeUnroll) return cudaErrorInvalidValue;
+    const long long nb = static_cast<long long>(R) * (K / g);
+    quantize_large_g_kernel<<<static_cast<unsigned>(nb), kLargeThreads, 0, st>>>(X, R, K, g, Q, S);
+  }
+  return cudaGetLastError();
+}
+bool quantize_supports_group(int g) {
+  const int gl = g / 32;
+  return ((gl & (gl - 1)) == 0 && gl <= 32) || gl <= kLargeThreads * kLargeUnroll;
+}
+cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, cudaStream_t st) {
+  const long long total = static_cast<long long>(R) * (K / 32);
+  pack_codes_kernel<<<static_cast<unsigned>((total + 255) / 256), 256, 0, st>>>(
+      codes, R, K, static_cast<uint8_t*>(q));
+  return cudaGetLastError();
+}
+cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, cudaStream_t st) {
+  const long long total = static_cast<long long>(R) * (K / 32);
+  unpack_codes_kernel<<<static_cast<unsigned>((total + 255) / 256), 256, 0, st>>>(
+      static_cast<const uint8_t*>(q), R, K, codes);
+  return cudaGetLastError();
+}
+cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st) {
+  const long long total = static_cast<long long>(round_up(R, kTileRows)) * G;
+  scales_from_natural_kernel<<<static_cast<unsigned>((total + 255) / 256), 256, 0, st>>>(
+      static_cast<const __half*>(nat), R, G, static_cast<__half*>(tiled));
+  return cudaGetLastError();
+}
+cudaError_t launch_scales_to_natural(const void* tiled, int R, int G, void* nat, cudaStream_t st) {
+  const long long total = static_cast<long long>(R) * G;
+  scales_to_natural_kernel<<<static_cast<unsigned>((total + 255) / 256), 256, 0, st>>>(
+      static_cast<const __half*>(tiled), R, G, static_cast<__half*>(nat));
+  return cudaGetLastError();
+}
+
+}  // namespace apex4

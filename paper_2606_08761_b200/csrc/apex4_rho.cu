@@ -1,0 +1,229 @@
+// apex4_rho.cu -- measures this GPU's own rho (Eq. 1-2; Table 1):
+// tensor-core throughput (dense INT8 tcgen05.mma kind::i8, the pipe the W4A4 path runs on, since
+// sm_100a has no 4-bit integer MMA) against CUDA-core throughput (FP32 FMA), plus the two other
+// rates that bound the dequant step a5: INT32->FP32 conversion and TMEM read bandwidth.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/apex4.h"
+#include "apex4_ptx.cuh"
+
+namespace apex4 {
+
+constexpr int kChains = 8;
+
+__global__ void __launch_bounds__(256) fma_rate_kernel(float* out, int iters, float b, float c) {
+  float a[kChains];
+#pragma unroll
+  for (int j = 0; j < kChains; ++j) a[j] = threadIdx.x * 0.001f + j;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < kChains; ++j) a[j] = fmaf(a[j], b, c);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int j = 0; j < kChains; ++j) s += a[j];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+__global__ void __launch_bounds__(256) fma2_rate_kernel(float* out, int iters, float b, float c) {
+  uint64_t a[kChains];
+  const uint64_t b2 = pack_f2(b, b), c2 = pack_f2(c, c);
+#pragma unroll
+  for (int j = 0; j < kChains; ++j) a[j] = pack_f2(threadIdx.x * 0.001f + j, 1.f + j);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < kChains; ++j) a[j] = fma2(a[j], b2, c2);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int j = 0; j < kChains; ++j) { float lo, hi; unpack_f2(a[j], lo, hi); s += lo + hi; }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+__global__ void __launch_bounds__(256) i2f_rate_kernel(float* out, int iters) {
+  int x[kChains];
+#pragma unroll
+  for (int j = 0; j < kChains; ++j) x[j] = threadIdx.x * 7 + j;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < kChains; ++j) x[j] = __float_as_int(__int2float_rn(x[j]));
+  }
+  int s = 0;
+#pragma unroll
+  for (int j = 0; j < kChains; ++j) s ^= x[j];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = __int_as_float(s);
+}
+
+// One CTA per SM: a single thread issues back-to-back 128x256x32 INT8 MMAs from resident shared
+// memory into two alternating TMEM accumulators; four warps then stream the accumulators out with
+// tcgen05.ld to time TMEM reads.
+constexpr int kMmaSmem = 1024 + 16384 + 32768 + 64;
+__global__ void __launch_bounds__(128, 1) mma_rate_kernel(int mma_iters, int ld_iters,
+                                                          long long* cycles_mma, long long* cycles_ld,
+                                                          uint32_t* sink) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* gen = smem_raw + (base - smem_u32(smem_raw));
+  for (int i = threadIdx.x; i < (16384 + 32768) / 4; i += blockDim.x)
+    reinterpret_cast<uint32_t*>(gen)[i] = 0x01010101u;
+  const uint32_t barA = base + 16384 + 32768, tptr = barA + 16;
+  if (threadIdx.x == 0) { mbar_init(barA, 1); fence_mbar_init(); }
+  fence_proxy_async_smem();
+  if (threadIdx.x < 32) tmem_alloc<512>(tptr);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(gen + 16384 + 32768 + 16);
+  long long t0 = 0, t1 = 0;
+  if (threadIdx.x == 0) {
+    constexpr uint32_t idesc = umma_idesc_i8(128, 256);
+    const uint64_t ad = umma_desc_sw128(base), bd = umma_desc_sw128(base + 16384);
+    t0 = clock64();
+    for (int it = 0; it < mma_iters; ++it) {
+#pragma unroll
+      for (int ks = 0; ks < 4; ++ks)
+        mma_i8_ss(tmem + (it & 1) * 256, ad + 2 * ks, bd + 2 * ks, idesc, ks ? 1u : 0u);
+    }
+    tc_commit(barA);
+    mbar_wait(barA, 0);
+    t1 = clock64();
+    cycles_mma[blockIdx.x] = t1 - t0;
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  {
+    const int warp = threadIdx.x >> 5;
+    const uint32_t taddr = tmem + (static_cast<uint32_t>(warp * 32) << 16);
+    uint32_t acc = 0;
+    const long long s0 = clock64();
+    for (int it = 0; it < ld_iters; ++it) {
+      uint32_t v[32];
+      tmem_ld_32x32(taddr + (it & 15) * 32, v);
+      tmem_ld_wait();
+#pragma unroll
+      for (int j = 0; j < 32; j += 8) acc ^= v[j];
+    }
+    const long long s1 = clock64();
+    if (threadIdx.x == 0) cycles_ld[blockIdx.x] = s1 - s0;
+    if (acc == 0x12345678u) sink[0] = acc;
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (threadIdx.x < 32) { tc_fence_after(); tmem_dealloc<512>(tmem); }
+}
+
+__global__ void clock_probe_kernel(long long* out) {
+  unsigned long long g0, g1;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
+  const long long c0 = clock64();
+  do {
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+  } while (g1 - g0 < 200000ull);   // 200 us
+  const long long c1 = clock64();
+  out[0] = c1 - c0;
+  out[1] = static_cast<long long>(g1 - g0);
+}
+
+static float time_ms(cudaEvent_t a, cudaEvent_t b) {
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, a, b);
+  return ms;
+}
+
+int measure_rho(double* out, cudaStream_t st) {
+  for (int i = 0; i < 8; ++i) out[i] = 0.0;
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  float* buf = nullptr;
+  long long* cyc = nullptr;
+  const int blocks = sms * 8, threads = 256;
+  if (cudaMalloc(&buf, sizeof(float) * blocks * threads) != cudaSuccess) return APEX4_ERR_CUDA;
+  if (cudaMalloc(&cyc, sizeof(long long) * (2 * sms + 2)) != cudaSuccess) { cudaFree(buf); return APEX4_ERR_CUDA; }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int iters = 4096;
+  int rc = APEX4_OK;
+  // FP32 FMA (scalar and packed)
+  double best_fma = 0, best_fma2 = 0, best_i2f = 0;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, st);
+    fma_rate_kernel<<<blocks, threads, 0, st>>>(buf, iters, 1.0001f, 0.5f);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { rc = APEX4_ERR_CUDA; break; }
+    double fl = 2.0 * blocks * threads * double(iters) * kChains / (time_ms(e0, e1) * 1e-3);
+    if (rep && fl > best_fma) best_fma = fl;
+    cudaEventRecord(e0, st);
+    fma2_rate_kernel<<<blocks, threads, 0, st>>>(buf, iters, 1.0001f, 0.5f);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { rc = APEX4_ERR_CUDA; break; }
+    fl = 4.0 * blocks * threads * double(iters) * kChains / (time_ms(e0, e1) * 1e-3);
+    if (rep && fl > best_fma2) best_fma2 = fl;
+    cudaEventRecord(e0, st);
+    i2f_rate_kernel<<<blocks, threads, 0, st>>>(buf, iters);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { rc = APEX4_ERR_CUDA; break; }
+    fl = 1.0 * blocks * threads * double(iters) * kChains / (time_ms(e0, e1) * 1e-3);
+    if (rep && fl > best_i2f) best_i2f = fl;
+  }
+  // INT8 tcgen05 MMA + TMEM read
+  double best_mma = 0, ld_bytes_per_clk = 0;
+  if (rc == APEX4_OK) {
+    cudaFuncSetAttribute(mma_rate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMmaSmem);
+    const int mma_iters = 8192, ld_iters = 4096;
+    for (int rep = 0; rep < 3; ++rep) {
+      cudaEventRecord(e0, st);
+      mma_rate_kernel<<<sms, 128, kMmaSmem, st>>>(mma_iters, ld_iters, cyc, cyc + sms,
+                                                  reinterpret_cast<uint32_t*>(buf));
+      cudaEventRecord(e1, st);
+      if (cudaEventSynchronize(e1) != cudaSuccess) { rc = APEX4_ERR_CUDA; break; }
+    }
+    if (rc == APEX4_OK) {
+      long long h[2];
+      cudaMemcpy(h, cyc, sizeof(long long), cudaMemcpyDeviceToHost);
+      cudaMemcpy(h + 1, cyc + sms, sizeof(long long), cudaMemcpyDeviceToHost);
+      // per-SM MACs per clock from the issuing thread's own cycle counter
+      const double macs = double(mma_iters) * 4 * 128.0 * 256.0 * 32.0;
+      out[6] = macs / double(h[0]);                               // INT8 MAC / clk / SM
+      ld_bytes_per_clk = double(ld_iters) * 4 * 4096.0 / double(h[1]);   // 4 warps x 4 KB per ld
+      out[7] = ld_bytes_per_clk;                                  // TMEM read B / clk / SM
+    }
+  }
+  // SM clock while idle-ish (context for the per-clock numbers)
+  double mhz = 0;
+  if (rc == APEX4_OK) {
+    clock_probe_kernel<<<1, 1, 0, st>>>(cyc + 2 * sms);
+    long long h[2];
+    if (cudaMemcpy(h, cyc + 2 * sms, 2 * sizeof(long long), cudaMemcpyDeviceToHost) == cudaSuccess && h[1] > 0)
+      mhz = double(h[0]) / double(h[1]) * 1e3;
+    else rc = APEX4_ERR_CUDA;
+  }
+  if (rc == APEX4_OK) {
+    // chip-level INT8 rate: time a long MMA-only launch with events
+    const int mma_iters = 32768;
+    cudaEventRecord(e0, st);
+    mma_rate_kernel<<<sms, 128, kMmaSmem, st>>>(mma_iters, 1, cyc, cyc + sms,
+                                                reinterpret_cast<uint32_t*>(buf));
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) == cudaSuccess) {
+      const double ops = 2.0 * sms * double(mma_iters) * 4 * 128.0 * 256.0 * 32.0;
+      best_mma = ops / (time_ms(e0, e1) * 1e-3);
+    } else rc = APEX4_ERR_CUDA;
+  }
+  out[0] = best_mma * 1e-12;                                  // INT8 TOPS (dense, kind::i8)
+  out[1] = (best_fma2 > best_fma ? best_fma2 : best_fma) * 1e-12;   // FP32 TFLOPS (best of FFMA / FFMA2)
+  out[2] = best_i2f * 1e-9;                                   // INT32->FP32 Gop/s
+  out[3] = out[1] > 0 ? out[0] / out[1] : 0;                  // rho = tensor ops / CUDA-core flops
+  out[4] = ld_bytes_per_clk * sms * mhz * 1e6 * 1e-9;         // TMEM read GB/s (chip)
+  out[5] = mhz;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(buf);
+  cudaFree(cyc);
+  return cudaGetLastError() == cudaSuccess ? rc : APEX4_ERR_CUDA;
+}
+
+}  // namespace apex4

@@ -1,0 +1,87 @@
+"""CPU-only checks of the boundary: libapex4.so builds/loads, exports every symbol include/apex4.h
+declares, and its host-side functions (no CUDA work) agree with the oracle's policy table."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from conftest import ROOT
+from oracle import apex4_oracle as O
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_2606_08761_b200 import build as B
+    B.build()
+    from paper_2606_08761_b200 import apex4
+    return apex4.lib()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "apex4.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(apex4_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(L):
+    names = declared_symbols()
+    assert "apex4_quantize_act" in names and "apex4_pack_weights" in names and "apex4_w4a4_gemm" in names
+    for n in names:
+        assert hasattr(L, n), n
+    from paper_2606_08761_b200 import apex4
+    assert set(apex4.EXPORTS) == set(names)
+
+
+def test_status_strings(L):
+    from paper_2606_08761_b200 import apex4
+    assert apex4.status_string(0) == "ok"
+    assert "workspace" in apex4.status_string(apex4.ERR_WORKSPACE)
+    assert "unknown" in apex4.status_string(99)
+
+
+def test_policy_table_matches_oracle(L):
+    from paper_2606_08761_b200 import apex4
+    K = 4096
+    for layer in range(10):
+        assert apex4.resolve_group_size(K, 128, apex4.GRAN_GROUP, layer) == 128
+        assert apex4.resolve_group_size(K, 0, apex4.GRAN_CHANNEL, layer) == K
+        assert apex4.resolve_group_size(K, 0, apex4.GRAN_MIXED, layer) == \
+            O.resolve_group_size(K, layer, O.POLICY_PAPER_MIX)
+        assert apex4.resolve_group_size(K, 0, apex4.GRAN_MIXED_G128, layer) == \
+            O.resolve_group_size(K, layer, O.POLICY_BASELINE_MIX)
+    assert apex4.resolve_group_size(K, 128, apex4.GRAN_GROUP, apex4.LAYER_DOWN) == \
+        O.resolve_group_size(K, O.LAYER_DOWN, O.POLICY_UNIFORM_G128)
+
+
+def test_argument_validation_without_gpu(L):
+    from paper_2606_08761_b200 import apex4
+    with pytest.raises(apex4.Apex4Error) as e:
+        apex4.resolve_group_size(4096, 48)            # not 32/64/multiple of 128
+    assert e.value.status == apex4.ERR_UNSUPPORTED_SHAPE
+    with pytest.raises(apex4.Apex4Error):
+        apex4.resolve_group_size(4000, 32)            # K % 128 != 0
+    with pytest.raises(apex4.Apex4Error):
+        apex4.resolve_group_size(4096, 128, 7)        # unknown gran
+    with pytest.raises(apex4.Apex4Error):
+        apex4.resolve_group_size(4096, 3072)          # does not divide K
+    assert apex4.packed_bytes(16, 512) == 4 * 8192    # 1 row tile x 4 k-blocks
+    assert apex4.packed_bytes(129, 512) == 8 * 8192
+    assert apex4.scale_elems(16, 512, 128) == 128 * 4
+    # null pointers are rejected before any CUDA call
+    assert L.apex4_w4a4_gemm(None, None, None, None, None, 0, 16, 256, 512, 128, 0, 0, None, 0, None) \
+        == apex4.ERR_INVALID_ARG
+    assert L.apex4_quantize_act(None, 16, 512, 128, 0, 0, None, None, None) == apex4.ERR_INVALID_ARG
+
+
+def test_dispatch_table(L):
+    from paper_2606_08761_b200 import apex4
+    swap, nc, splits, kbps = apex4.debug_get_dispatch(16, 8192, 8192, 128)
+    assert swap == 1 and nc == 16 and splits >= 2 and kbps * splits >= 64
+    swap, nc, splits, kbps = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
+    assert (swap, nc, splits, kbps) == (0, 256, 1, 64)
+    # per-channel: the k range cannot be split inside a group
+    swap, nc, splits, kbps = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
+    assert splits == 1 and kbps == 64
+    assert apex4.workspace_bytes(8192, 8192, 8192, 128) == 0
+    assert apex4.workspace_bytes(16, 8192, 8192, 128) == 4096 * 4 + 16 * 8192 * 4

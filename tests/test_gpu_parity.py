@@ -1,0 +1,243 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs.  Bars: bit-exact INT4 codes, FP16 scales and per-group INT32 sums; outputs within
+|y - Y64| <= 1e-3 |Y64| + (G+2) 2^-23 T (+ 2^-24 for FP16 output) -- reading R12 of DESIGN.md."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import apex4_oracle as O
+from paper_2606_08761_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def A():
+    from paper_2606_08761_b200 import apex4
+    apex4.lib()
+    assert torch.cuda.is_available()
+    yield apex4
+    apex4.debug_set_dispatch(-1, -1, -1)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_quantize(A, X, g, weights=False):
+    """-> (q_packed, s_tiled, codes int8 numpy [R,K], scales fp16 numpy [R,G])"""
+    R, K = X.shape
+    fn = A.pack_weights if weights else A.quantize_act
+    q, s, g_res = fn(dev(X), g)
+    assert g_res == g
+    codes = A.unpack_codes(q, R, K).cpu().numpy()
+    scales = A.scales_to_natural(s, R, K // g).cpu().numpy()
+    return q, s, codes, scales
+
+
+def check_output(Y_gpu, Y64, T, G, f16):
+    tol = O.output_tolerance(Y64, T, G, f16)
+    err = np.abs(Y_gpu.astype(np.float64) - Y64)
+    bad = err > tol
+    assert not bad.any(), (int(bad.sum()), float((err / np.maximum(tol, 1e-300)).max()),
+                           np.argwhere(bad)[:5].tolist())
+
+
+# ------------------------------------------------------------------------------- quantizer (a0/a1)
+@pytest.mark.parametrize("M,K,g", [(16, 512, 128), (16, 512, 32), (16, 512, 64), (16, 512, 256),
+                                   (16, 512, 512), (1, 128, 128), (13, 1024, 1024), (130, 384, 128),
+                                   (257, 2048, 2048), (5, 11008, 11008), (3, 28672, 28672),
+                                   (300, 4096, 128)])
+def test_quantizer_bit_exact(A, M, K, g):
+    X = inputs.make_activations(M, K, seed=17 + M, fixed_outliers=(K == 512))
+    qo, so = O.quantize(X, g)
+    _, _, codes, scales = gpu_quantize(A, X, g)
+    assert np.array_equal(scales.view(np.uint16), so.view(np.uint16))
+    assert np.array_equal(codes, qo)
+
+
+def test_quantizer_weights_config0(A):
+    X, W, g = inputs.config0()
+    qo, so = O.quantize(W, g)
+    _, _, codes, scales = gpu_quantize(A, W, g, weights=True)
+    assert np.array_equal(scales.view(np.uint16), so.view(np.uint16))
+    assert np.array_equal(codes, qo)
+
+
+def test_quantizer_exhaustive_fp16_inputs(A):
+    """Every finite FP16 bit pattern through the GPU quantizer, for a set of group scales that
+    includes FP16-subnormal scales (R4/R5), compared with the oracle element by element."""
+    allb = np.arange(0x10000, dtype=np.uint32).astype(np.uint16)
+    finite = allb[((allb >> 10) & 0x1F) != 0x1F].view(np.float16)
+    mags = np.abs(finite.astype(np.float64))
+    u = 2.0 ** -24
+    for amax in (1.0, 7.0, 20.0, 0.0200042724609375, 65504.0, 3 * u, 10 * u, 11 * u, 100 * u, 0.33):
+        cand = finite[mags <= amax]
+        n = (cand.size + 1 + 127) // 128 * 128
+        X = np.zeros((1, n), dtype=np.float16)
+        X[0, :cand.size] = cand
+        X[0, cand.size] = np.float16(amax)
+        qo, so = O.quantize(X, n)
+        _, _, codes, scales = gpu_quantize(A, X, n)
+        assert np.array_equal(scales.view(np.uint16), so.view(np.uint16)), amax
+        assert np.array_equal(codes, qo), amax
+    # many groups with different scales in one launch (g = 32): random magnitudes incl. tiny ones
+    rng = np.random.default_rng(5)
+    X = (rng.standard_normal((64, 1024)) * np.exp2(rng.integers(-26, 12, size=(64, 1024 // 32)).repeat(32, 1))
+         ).astype(np.float16)
+    qo, so = O.quantize(X, 32)
+    _, _, codes, scales = gpu_quantize(A, X, 32)
+    assert np.array_equal(scales.view(np.uint16), so.view(np.uint16))
+    assert np.array_equal(codes, qo)
+
+
+def test_pack_unpack_roundtrip_and_scale_layout(A):
+    rng = np.random.default_rng(9)
+    codes = rng.integers(-8, 8, size=(200, 640)).astype(np.int8)
+    q = A.pack_codes(dev(codes))
+    assert q.numel() == A.packed_bytes(200, 640)
+    assert np.array_equal(A.unpack_codes(q, 200, 640).cpu().numpy(), codes)
+    s = rng.standard_normal((200, 5)).astype(np.float16)
+    t = A.scales_from_natural(dev(s))
+    assert np.array_equal(A.scales_to_natural(t, 200, 5).cpu().numpy().view(np.uint16), s.view(np.uint16))
+
+
+# ------------------------------------------------------------------------------- GEMM (a2..a7)
+def run_gemm_case(A, M, N, K, g, seed, fixed=False, out_f32=False, sums="all", dispatch=None):
+    X, W = inputs.make_gemm_inputs(M, N, K, seed, fixed_outliers=fixed)
+    ref = O.w4a4_linear(X, W, g)
+    G = K // g
+    if dispatch is not None:
+        A.debug_set_dispatch(*dispatch)
+    try:
+        qA, sA, _ = A.quantize_act(dev(X), g)
+        qW, sW, _ = A.pack_weights(dev(W), g)
+        Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g,
+                        out_dtype=torch.float32 if out_f32 else torch.float16)
+        # a second call on the same (self-cleaning) workspace must give the same answer
+        ws = A.make_workspace(M, N, K, g)
+        Y2 = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=Y.dtype, workspace=ws)
+        Y3 = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=Y.dtype, workspace=ws)
+        if sums == "all":
+            P = A.debug_group_sums(qA, qW, M, N, K, g).cpu().numpy()
+            assert np.array_equal(P, O.group_sums(ref["qA"], ref["qW"], g))
+        elif sums is not None:
+            m0, m1, n0, n1 = sums
+            P = A.debug_group_sums(qA, qW, M, N, K, g, m0=m0, m1=m1, n0=n0, n1=n1).cpu().numpy()
+            assert np.array_equal(P, O.group_sums(ref["qA"][m0:m1], ref["qW"][n0:n1], g))
+        torch.cuda.synchronize()
+    finally:
+        A.debug_set_dispatch(-1, -1, -1)
+    for y in (Y, Y2, Y3):
+        check_output(y.cpu().numpy(), ref["Y64"], ref["T"], G, not out_f32)
+    if ws is not None:
+        assert int(ws.count_nonzero()) == 0      # workspace left zero-filled
+    return ref
+
+
+def test_gemm_config0(A):
+    """BASELINE.json config 0: M=16, N=256, K=512, g=128, seed 0 -- every output, every group sum."""
+    X, W, g = inputs.config0()
+    assert X.shape == (16, 512) and W.shape == (256, 512)
+    run_gemm_case(A, 16, 256, 512, 128, seed=0, fixed=True)
+
+
+@pytest.mark.parametrize("g", [32, 64, 128, 256, 512])
+@pytest.mark.parametrize("dispatch", [(0, 128, 1), (0, 256, 1), (1, 16, 1), (1, 16, 2), (0, 128, 2),
+                                      (1, 64, 1), (1, 32, 4)])
+def test_gemm_config0_all_dispatches(A, g, dispatch):
+    """Same problem through both orientations, several tile widths and split-K factors."""
+    run_gemm_case(A, 16, 256, 512, g, seed=0, fixed=True, dispatch=dispatch)
+
+
+@pytest.mark.parametrize("M,N,K,g", [(1, 256, 512, 128), (4, 264, 1024, 128), (17, 136, 384, 32),
+                                     (64, 512, 1024, 64), (100, 384, 2048, 2048), (130, 520, 1024, 128),
+                                     (257, 768, 1536, 512), (300, 1000, 512, 128), (256, 2048, 4096, 128)])
+def test_gemm_ragged_and_multi_tile(A, M, N, K, g):
+    run_gemm_case(A, M, N, K, g, seed=100 + M)
+
+
+def test_gemm_f32_output(A):
+    run_gemm_case(A, 40, 256, 1024, 128, seed=3, out_f32=True)
+    run_gemm_case(A, 200, 512, 1024, 128, seed=4, out_f32=True)
+
+
+def test_gemm_all_ones_closed_form(A):
+    """P3: X = W = 1 -> every code 7, P = 49 g, Y = 49 K (585/4096)^2 for every g."""
+    for (M, N, K) in [(16, 256, 512), (150, 384, 4096)]:
+        X = np.ones((M, K), dtype=np.float16)
+        W = np.ones((N, K), dtype=np.float16)
+        for g in (32, 128, K):
+            qA, sA, _ = A.quantize_act(dev(X), g)
+            qW, sW, _ = A.pack_weights(dev(W), g)
+            Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g).cpu().numpy()
+            want = np.float16(49.0 * K * (585.0 / 4096.0) ** 2)
+            assert np.all(Y == want), (M, N, K, g)
+            P = A.debug_group_sums(qA, qW, M, N, K, g, m1=min(M, 8), n1=16).cpu().numpy()
+            assert np.all(P == 49 * g)
+
+
+def test_gemm_minus8_codes_headroom(A):
+    """R5: all-(-8) codes injected through apex4_pack_codes: P = 64 g, exact up to per-channel K."""
+    M, N, K = 8, 128, 4096
+    cA = np.full((M, K), -8, dtype=np.int8)
+    cW = np.full((N, K), -8, dtype=np.int8)
+    qA, qW = A.pack_codes(dev(cA)), A.pack_codes(dev(cW))
+    for g in (32, 128, K):
+        P = A.debug_group_sums(qA, qW, M, N, K, g).cpu().numpy()
+        assert np.all(P == 64 * g)
+    g = 128
+    sA = A.scales_from_natural(dev(np.full((M, K // g), 0.5, dtype=np.float16)))
+    sW = A.scales_from_natural(dev(np.full((N, K // g), 0.25, dtype=np.float16)))
+    Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=torch.float32).cpu().numpy()
+    assert np.all(Y == 64.0 * K * 0.125)
+
+
+def test_gemm_sampled_large(A):
+    """A Llama-2-7B shaped layer (config 1, O-proj) at M=2048: sampled rows x all columns and all rows
+    x sampled columns against the oracle, group sums bit-exact on a window per tile corner."""
+    M, N, K, g = 2048, 4096, 4096, 128
+    X, W = inputs.make_gemm_inputs(M, N, K, inputs.config_seed(1, 1), fixed_outliers=True)
+    qA, sA, _ = A.quantize_act(dev(X), g)
+    qW, sW, _ = A.pack_weights(dev(W), g)
+    Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g).cpu().numpy()
+    rows = inputs.sample_rows(M, 1)
+    cols = inputs.sample_rows(N, 2)
+    qa, sa = O.quantize(X, g)
+    qw, sw = O.quantize(W, g)
+    Y64, T = O.dequant_gemm(qa[rows], sa[rows], qw, sw, g)
+    check_output(Y[rows], Y64, T, K // g, True)
+    Y64, T = O.dequant_gemm(qa, sa, qw[cols], sw[cols], g)
+    check_output(Y[:, cols], Y64, T, K // g, True)
+    for (m0, n0) in [(0, 0), (120, 250), (2040, 4088), (1000, 2040)]:
+        P = A.debug_group_sums(qA, qW, M, N, K, g, m0=m0, m1=m0 + 8, n0=n0, n1=n0 + 8).cpu().numpy()
+        assert np.array_equal(P, O.group_sums(qa[m0:m0 + 8], qw[n0:n0 + 8], g))
+
+
+def test_linear_host_matches_device_path(A):
+    M, N, K, g = 16, 256, 512, 128
+    X, W, _ = inputs.config0()
+    ref = O.w4a4_linear(X, W, g)
+    qW, sW, _ = A.pack_weights(dev(W), g)
+    xh = torch.from_numpy(X).pin_memory()
+    yh = torch.empty((M, N), dtype=torch.float16).pin_memory()
+    A.w4a4_linear_host(xh, qW, sW, yh, N, g)
+    torch.cuda.synchronize()
+    check_output(yh.numpy(), ref["Y64"], ref["T"], K // g, True)
+
+
+def test_error_codes_on_device(A):
+    x = torch.zeros((16, 512), dtype=torch.float16, device="cuda")
+    with pytest.raises(A.Apex4Error) as e:
+        A.quantize_act(x, 48)
+    assert e.value.status == A.ERR_UNSUPPORTED_SHAPE
+    q, s, _ = A.quantize_act(x, 128)
+    with pytest.raises(A.Apex4Error) as e:     # split-K dispatch without a workspace
+        A.lib().apex4_debug_set_dispatch(1, 16, 2)
+        try:
+            st = A.lib().apex4_w4a4_gemm(q.data_ptr(), s.data_ptr(), q.data_ptr(), s.data_ptr(), x.data_ptr(),
+                                         0, 16, 128, 512, 128, 0, 0, None, 0, None)
+            A._check(st, "gemm")
+        finally:
+            A.debug_set_dispatch(-1, -1, -1)
+    assert e.value.status == A.ERR_WORKSPACE
