@@ -73,10 +73,14 @@ def test_quantizer_exhaustive_fp16_inputs(A):
     u = 2.0 ** -24
     for amax in (1.0, 7.0, 20.0, 0.0200042724609375, 65504.0, 3 * u, 10 * u, 11 * u, 100 * u, 0.33):
         cand = finite[mags <= amax]
-        n = (cand.size + 1 + 127) // 128 * 128
-        X = np.zeros((1, n), dtype=np.float16)
-        X[0, :cand.size] = cand
-        X[0, cand.size] = np.float16(amax)
+        n = 32768                                   # per-channel rows of the maximum supported K
+        per = n - 1
+        rows = (cand.size + per - 1) // per
+        X = np.zeros((rows, n), dtype=np.float16)
+        for r in range(rows):
+            part = cand[r * per:(r + 1) * per]
+            X[r, :part.size] = part
+            X[r, n - 1] = np.float16(amax)          # every row has the same absmax -> the same scale
         qo, so = O.quantize(X, n)
         _, _, codes, scales = gpu_quantize(A, X, n)
         assert np.array_equal(scales.view(np.uint16), so.view(np.uint16)), amax
