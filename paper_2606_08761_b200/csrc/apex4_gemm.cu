@@ -191,21 +191,27 @@ __global__ void __launch_bounds__(GemmCfg<NC>::kThreads, 1) w4a4_gemm_kernel(con
       mbar_wait(bar(bPkFull + s), phs);
       mbar_wait(bar(bI8Empty + t), pht ^ 1);
       const uint8_t* pk = smem_gen + offPk + s * Cfg::kPkStageBytes;
-      uint8_t* i8 = smem_gen + offI8 + t * Cfg::kI8StageBytes;
+      const uint32_t pk_addr = smem_base + offPk + s * Cfg::kPkStageBytes;
+      const uint32_t i8_addr = smem_base + offI8 + t * Cfg::kI8StageBytes;
       // packed byte offset o -> INT8 byte offsets 2o (lo nibbles) and 2o+16 (hi nibbles); the R blob
       // and the C tile are adjacent in both buffers, so one linear loop covers both
       constexpr int kChunks = (Cfg::kPkRBytes + Cfg::kCPackedBytes) / 16;
 #pragma unroll 4
       for (int ci = w; ci < kChunks; ci += 128) {
-        const uint4 v = *reinterpret_cast<const uint4*>(pk + ci * 16);
-        uint4 lo, hi;
-        lo.x = (v.x << 4) & 0xF0F0F0F0u; hi.x = v.x & 0xF0F0F0F0u;
-        lo.y = (v.y << 4) & 0xF0F0F0F0u; hi.y = v.y & 0xF0F0F0F0u;
-        lo.z = (v.z << 4) & 0xF0F0F0F0u; hi.z = v.z & 0xF0F0F0F0u;
-        lo.w = (v.w << 4) & 0xF0F0F0F0u; hi.w = v.w & 0xF0F0F0F0u;
-        uint8_t* dst = i8 + ci * 32;
-        *reinterpret_cast<uint4*>(dst + flip) = flip ? hi : lo;
-        *reinterpret_cast<uint4*>(dst + (16 - flip)) = flip ? lo : hi;
+        uint32_t v0, v1, v2, v3;
+        lds128(pk_addr + ci * 16, v0, v1, v2, v3);
+        const uint32_t l0 = (v0 << 4) & 0xF0F0F0F0u, h0 = v0 & 0xF0F0F0F0u;
+        const uint32_t l1 = (v1 << 4) & 0xF0F0F0F0u, h1 = v1 & 0xF0F0F0F0u;
+        const uint32_t l2 = (v2 << 4) & 0xF0F0F0F0u, h2 = v2 & 0xF0F0F0F0u;
+        const uint32_t l3 = (v3 << 4) & 0xF0F0F0F0u, h3 = v3 & 0xF0F0F0F0u;
+        const uint32_t dst = i8_addr + ci * 32;
+        if (flip) {   // warp-divergence free in effect: both sides are two 128-bit stores
+          sts128(dst + 16, h0, h1, h2, h3);
+          sts128(dst, l0, l1, l2, l3);
+        } else {
+          sts128(dst, l0, l1, l2, l3);
+          sts128(dst + 16, h0, h1, h2, h3);
+        }
       }
       fence_proxy_async_smem();
       mbar_arrive(bar(bI8Full + t));
