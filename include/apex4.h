@@ -6,8 +6,9 @@
  *   Eq. 8  group-dequantised GEMM
  *        Y[m,n] = sum_g sA[m,g] * sW[n,g] * (sum_{k in g} qA[m,k] * qW[n,k])
  *        exact INT32 partial sums per K-group on the tensor cores (tcgen05.mma kind::i8,
- *        operands widened INT4->INT8 in shared memory because sm_100a has no 4-bit integer
- *        MMA kind), INT32->FP32 + scale multiply on the CUDA cores, FP32 accumulation.
+ *        operands widened INT4->INT8 on chip because sm_100a has no 4-bit integer MMA kind:
+ *        weights in registers -> TMEM, activations shared -> shared memory), INT32->FP32 + scale
+ *        multiply on the CUDA cores, FP32 accumulation.
  *   3.2.2  granularity: uniform g, per-channel (g = K), mixed policy.
  *
  * Conventions
@@ -26,6 +27,9 @@
  *                     occupies 64 bytes and its 16-byte chunks / nibbles are permuted so that the
  *                     in-kernel widening lands directly in the 128B-swizzled UMMA operand layout
  *                     (see csrc/apex4_layout.cuh).  apex4_unpack_codes inverts it.
+ *                     "PW4" (weights): same blobs and sizes, a different permutation inside a row
+ *                     (the weights are widened in registers and stored to TMEM).  A buffer packed
+ *                     as one operand kind must be used as that kind.
  *       scales        "ST16": FP16, tile-major [Rp/128][G][128], G = K/g: element (r, gamma) at
  *                     ((r/128) * G + gamma) * 128 + r % 128.  apex4_scales_to_natural inverts it.
  */
@@ -65,6 +69,9 @@ typedef enum {
 
 typedef enum { APEX4_OUT_F16 = 0, APEX4_OUT_F32 = 1 } apex4_out;
 
+/* which GEMM operand a packed-code buffer belongs to (selects the PT4 or the PW4 layout) */
+typedef enum { APEX4_OPERAND_ACT = 0, APEX4_OPERAND_WEIGHT = 1 } apex4_operand;
+
 /* ---- host-side queries (no CUDA work) ------------------------------------------------------- */
 
 /* Group size a call with these arguments runs at, or a negative apex4_status on invalid input.
@@ -87,22 +94,25 @@ int apex4_quantize_act(const void* x_f16, int M, int K, int group_size, int gran
                        void* qA_packed, void* sA_f16, void* stream);
 
 /* ---- a0: offline weight quantize + pack (Eq. 7) --------------------------- */
-/* w_f16 [N,K] FP16 -> qW_packed (PT4) + sW_f16 (ST16). Same arithmetic as the activation quantizer. */
+/* w_f16 [N,K] FP16 -> qW_packed (PW4) + sW_f16 (ST16). Same arithmetic as the activation quantizer. */
 int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran, int layer,
                        void* qW_packed, void* sW_f16, void* stream);
 /* Offline-calibrated path (Alg. 1 output): codes [R,K] int8 in [-8,7] (row-major)
- * -> PT4.  Values outside [-8,7] are taken modulo 16 (low nibble). */
-int apex4_pack_codes(const int8_t* codes, int R, int K, void* q_packed, void* stream);
+ * -> PT4 (operand = APEX4_OPERAND_ACT) or PW4 (APEX4_OPERAND_WEIGHT).  Values outside [-8,7] are
+ * taken modulo 16 (low nibble). */
+int apex4_pack_codes(const int8_t* codes, int R, int K, int operand, void* q_packed, void* stream);
 /* natural FP16 scales [R,G] row-major -> ST16 (padding rows zero-filled), and back. */
 int apex4_scales_from_natural(const void* s_nat_f16, int R, int G, void* s_tiled_f16, void* stream);
 int apex4_scales_to_natural(const void* s_tiled_f16, int R, int G, void* s_nat_f16, void* stream);
-/* PT4 -> codes [R,K] int8 (verification twin of the packers; works for activations and weights). */
-int apex4_unpack_codes(const void* q_packed, int R, int K, int8_t* codes, void* stream);
+/* PT4 / PW4 (per `operand`) -> codes [R,K] int8 (verification twin of the packers). */
+int apex4_unpack_codes(const void* q_packed, int R, int K, int operand, int8_t* codes, void* stream);
 
 /* ---- a2..a7: the W4A4 group-dequant GEMM (Eq. 8) ----------------------------- */
 /* Y [M,N] (FP16 or FP32 per out_dtype) = sum_g sA sW P_g.  qA/sA from apex4_quantize_act, qW/sW
  * from apex4_pack_weights, both at the same resolved group size (G_a = G_w).
- * workspace: apex4_workspace_bytes() bytes (may be NULL when that is 0). */
+ * workspace: apex4_workspace_bytes() bytes (may be NULL when that is 0); it is needed when the K loop
+ * of an output tile is shared between CTAs (a6: decode-sized M, or a tile count
+ * that does not fill the 148 SMs evenly). */
 int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
                     const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
                     int gran, int layer, void* workspace, size_t workspace_bytes, void* stream);

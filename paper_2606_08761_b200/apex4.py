@@ -22,6 +22,7 @@ GRAN_GROUP, GRAN_CHANNEL, GRAN_MIXED, GRAN_MIXED_G128 = range(4)
 (LAYER_OTHER, LAYER_Q, LAYER_K, LAYER_V, LAYER_QKV, LAYER_O, LAYER_GATE, LAYER_UP, LAYER_GATE_UP,
  LAYER_DOWN) = range(10)
 OUT_F16, OUT_F32 = 0, 1
+OPERAND_ACT, OPERAND_WEIGHT = 0, 1
 
 EXPORTS = (
     "apex4_resolve_group_size", "apex4_packed_bytes", "apex4_scale_elems", "apex4_workspace_bytes",
@@ -66,8 +67,8 @@ def lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
         f.restype = c_int
-    L.apex4_pack_codes.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p]
-    L.apex4_unpack_codes.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p]
+    L.apex4_pack_codes.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
+    L.apex4_unpack_codes.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
     L.apex4_scales_from_natural.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p]
     L.apex4_scales_to_natural.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p]
     L.apex4_w4a4_gemm.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int,
@@ -149,22 +150,25 @@ def quantize_act(x, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, q=None, 
 
 
 def pack_weights(w, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, q=None, s=None):
-    """apex4_pack_weights: W[N,K] fp16 -> (qW PT4, sW ST16, g)."""
+    """apex4_pack_weights: W[N,K] fp16 -> (qW PW4, sW ST16, g)."""
     return _quantize("apex4_pack_weights", w, group_size, gran, layer, q, s)
 
 
-def pack_codes(codes: torch.Tensor) -> torch.Tensor:
+def pack_codes(codes: torch.Tensor, operand: int) -> torch.Tensor:
+    """apex4_pack_codes: int8 codes [R,K] -> PT4 (OPERAND_ACT) or PW4 (OPERAND_WEIGHT)."""
     _dev(codes, torch.int8, "apex4_pack_codes")
     R, K = codes.shape
     q = torch.empty(packed_bytes(R, K), dtype=torch.uint8, device=codes.device)
-    _check(lib().apex4_pack_codes(codes.data_ptr(), R, K, q.data_ptr(), _stream()), "apex4_pack_codes")
+    _check(lib().apex4_pack_codes(codes.data_ptr(), R, K, operand, q.data_ptr(), _stream()),
+           "apex4_pack_codes")
     return q
 
 
-def unpack_codes(q: torch.Tensor, R: int, K: int) -> torch.Tensor:
+def unpack_codes(q: torch.Tensor, R: int, K: int, operand: int) -> torch.Tensor:
     _dev(q, torch.uint8, "apex4_unpack_codes")
     codes = torch.empty((R, K), dtype=torch.int8, device=q.device)
-    _check(lib().apex4_unpack_codes(q.data_ptr(), R, K, codes.data_ptr(), _stream()), "apex4_unpack_codes")
+    _check(lib().apex4_unpack_codes(q.data_ptr(), R, K, operand, codes.data_ptr(), _stream()),
+           "apex4_unpack_codes")
     return codes
 
 
@@ -248,11 +252,13 @@ def measure_rho() -> dict:
     return dict(zip(keys, [float(v) for v in out]))
 
 
-def debug_set_dispatch(swap: int = -1, nc: int = -1, splits: int = -1) -> None:
-    lib().apex4_debug_set_dispatch(swap, nc, splits)
+def debug_set_dispatch(nt: int = -1, split: int = -1, grid: int = -1) -> None:
+    """Test hook: force the token-tile width (16..256), stream-K (0/1) and the grid size."""
+    lib().apex4_debug_set_dispatch(nt, split, grid)
 
 
 def debug_get_dispatch(M, N, K, g) -> Tuple[int, int, int, int]:
+    """-> (token-tile width, stream-K flag, grid size, k units per tile)"""
     out = (ctypes.c_int * 4)()
     lib().apex4_debug_get_dispatch(M, N, K, g, out)
     return tuple(int(v) for v in out)

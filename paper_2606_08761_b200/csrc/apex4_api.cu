@@ -1,5 +1,5 @@
 // apex4_api.cu -- the C ABI of include/apex4.h: argument validation, granularity policy (a8),
-// dispatch between the normal and the swapped/split-K orientation of the GEMM kernel.
+// choice of token-tile width and work distribution (whole tiles / stream-K) for the GEMM kernel.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>
@@ -9,10 +9,11 @@
 #include "apex4_layout.cuh"
 
 namespace apex4 {
-cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, cudaStream_t st);
+cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, int weights,
+                            cudaStream_t st);
 bool quantize_supports_group(int g);
-cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, cudaStream_t st);
-cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, cudaStream_t st);
+cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, int weights, cudaStream_t st);
+cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, int weights, cudaStream_t st);
 cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st);
 cudaError_t launch_scales_to_natural(const void* tiled, int R, int G, void* nat, cudaStream_t st);
 int measure_rho(double* out, cudaStream_t st);
@@ -21,8 +22,6 @@ int measure_rho(double* out, cudaStream_t st);
 using namespace apex4;
 
 namespace {
-
-constexpr int kCounterInts = 4096;   // split-K arrival counters live at the front of the workspace
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -62,44 +61,48 @@ int resolve_g(int K, int group_size, int gran, int layer) {
 }
 
 struct Dispatch {
-  int swap, nc, splits, kb_per_split;
+  int nt;      // token-tile width
+  int bias;    // magic-biased accumulators (g <= 128)
+  int split;   // stream-K work distribution (needs the workspace)
+  int grid;
+  int upt, kbu, tiles_m, tiles_n;
 };
 
 // test hook (apex4_debug_set_dispatch): -1 = automatic
-int g_force_swap = -1, g_force_nc = -1, g_force_splits = -1;
+int g_force_nt = -1, g_force_split = -1, g_force_grid = -1;
 
 Dispatch choose_dispatch(int M, int N, int K, int g) {
   Dispatch d;
   const int KB = K / kBlockK;
-  const int kbpg = g > kBlockK ? g / kBlockK : 1;
-  const int units = KB / kbpg;   // indivisible k units (whole groups)
-  d.swap = (g_force_swap >= 0) ? g_force_swap : (M <= 64 ? 1 : 0);
-  const int Rn = d.swap ? N : M, Cn = d.swap ? M : N;
-  if (g_force_nc > 0) d.nc = g_force_nc;
-  else if (Cn <= 16) d.nc = 16;
-  else if (Cn <= 32) d.nc = 32;
-  else if (Cn <= 64) d.nc = 64;
-  else if (Cn <= 128) d.nc = 128;
-  else d.nc = 256;
-  const int r_tiles = (Rn + kTileRows - 1) / kTileRows;
-  int c_tiles = (Cn + d.nc - 1) / d.nc;
-  if (g_force_nc <= 0 && d.nc == 256 && r_tiles * c_tiles < 148 && Cn > 128) {
-    d.nc = 128;   // more, smaller tiles when the grid would not fill the chip
-    c_tiles = (Cn + 127) / 128;
-  }
-  const int tiles = r_tiles * c_tiles;
-  int splits = 1;
-  if (g_force_splits > 0) splits = g_force_splits;
-  else if (tiles < 148) {
-    const int slots = d.nc <= 64 ? 296 : 148;   // small-NC kernels fit two CTAs per SM
-    splits = slots / tiles;
-  }
-  if (splits > units) splits = units;
-  if (splits < 1) splits = 1;
-  const int units_per = (units + splits - 1) / splits;
-  d.kb_per_split = units_per * kbpg;
-  d.splits = (units + units_per - 1) / units_per;
+  d.kbu = g > kBlockK ? g / kBlockK : 1;   // indivisible k unit: a whole group, at least a k-block
+  d.upt = KB / d.kbu;
+  d.bias = g <= kBlockK;
+  if (g_force_nt > 0) d.nt = g_force_nt;
+  else if (M <= 16) d.nt = 16;
+  else if (M <= 32) d.nt = 32;
+  else if (M <= 64) d.nt = 64;
+  else if (M <= 128) d.nt = 128;
+  else d.nt = 256;
+  d.tiles_m = (M + d.nt - 1) / d.nt;
+  d.tiles_n = (N + kTileRows - 1) / kTileRows;
+  const long long tiles = static_cast<long long>(d.tiles_m) * d.tiles_n;
+  const long long units = tiles * d.upt;
+  const int sms = g_force_grid > 0 ? g_force_grid : gemm_max_ctas();
+  d.grid = static_cast<int>(units < sms ? units : sms);
+  // whole tiles per CTA when the last wave is reasonably full, stream-K otherwise
+  const long long waves = (tiles + d.grid - 1) / d.grid;
+  const double eff = static_cast<double>(tiles) / static_cast<double>(waves * d.grid);
+  d.split = (g_force_split >= 0) ? g_force_split : (eff < 0.93 ? 1 : 0);
+  if (d.upt == 1) d.split = 0;                      // nothing to split
+  if (!d.split && tiles < d.grid) d.grid = static_cast<int>(tiles);
   return d;
+}
+
+size_t counters_bytes(const Dispatch& d) {
+  return (static_cast<size_t>(d.tiles_m) * d.tiles_n * 4 + 255) / 256 * 256;
+}
+size_t workspace_need(const Dispatch& d, int M, int N) {
+  return d.split ? counters_bytes(d) + static_cast<size_t>(M) * N * 4 : 0;
 }
 
 int validate_gemm_shape(int M, int N, int K) {
@@ -142,13 +145,11 @@ size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int 
   if (validate_gemm_shape(M, N, K) != APEX4_OK) return 0;
   const int g = resolve_g(K, group_size, gran, layer);
   if (g < 0) return 0;
-  const Dispatch d = choose_dispatch(M, N, K, g);
-  if (d.splits <= 1) return 0;
-  return static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4;
+  return workspace_need(choose_dispatch(M, N, K, g), M, N);
 }
 
 static int quantize_common(const void* x, int R, int K, int group_size, int gran, int layer, void* q,
-                           void* s, void* stream) {
+                           void* s, int weights, void* stream) {
   if (!x || !q || !s || R < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
   if (K > 32768) return APEX4_ERR_UNSUPPORTED_SHAPE;
   const int g = resolve_g(K, group_size, gran, layer);
@@ -156,37 +157,39 @@ static int quantize_common(const void* x, int R, int K, int group_size, int gran
   if (!aligned16(x) || !aligned16(q) || !aligned16(s)) return APEX4_ERR_ALIGNMENT;
   const int a = check_arch();
   if (a != APEX4_OK) return a;
-  return launch_quantize(x, R, K, g, q, s, static_cast<cudaStream_t>(stream)) == cudaSuccess
+  return launch_quantize(x, R, K, g, q, s, weights, static_cast<cudaStream_t>(stream)) == cudaSuccess
              ? APEX4_OK
              : APEX4_ERR_CUDA;
 }
 
 int apex4_quantize_act(const void* x_f16, int M, int K, int group_size, int gran, int layer,
                        void* qA_packed, void* sA_f16, void* stream) {
-  return quantize_common(x_f16, M, K, group_size, gran, layer, qA_packed, sA_f16, stream);
+  return quantize_common(x_f16, M, K, group_size, gran, layer, qA_packed, sA_f16, 0, stream);
 }
 int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran, int layer,
                        void* qW_packed, void* sW_f16, void* stream) {
-  return quantize_common(w_f16, N, K, group_size, gran, layer, qW_packed, sW_f16, stream);
+  return quantize_common(w_f16, N, K, group_size, gran, layer, qW_packed, sW_f16, 1, stream);
 }
 
-int apex4_pack_codes(const int8_t* codes, int R, int K, void* q_packed, void* stream) {
+int apex4_pack_codes(const int8_t* codes, int R, int K, int operand, void* q_packed, void* stream) {
   if (!codes || !q_packed || R < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
+  if (operand != APEX4_OPERAND_ACT && operand != APEX4_OPERAND_WEIGHT) return APEX4_ERR_INVALID_ARG;
   if (K % kBlockK != 0) return APEX4_ERR_UNSUPPORTED_SHAPE;
   if (!aligned16(codes) || !aligned16(q_packed)) return APEX4_ERR_ALIGNMENT;
   const int a = check_arch();
   if (a != APEX4_OK) return a;
-  return launch_pack_codes(codes, R, K, q_packed, static_cast<cudaStream_t>(stream)) == cudaSuccess
+  return launch_pack_codes(codes, R, K, q_packed, operand, static_cast<cudaStream_t>(stream)) == cudaSuccess
              ? APEX4_OK
              : APEX4_ERR_CUDA;
 }
-int apex4_unpack_codes(const void* q_packed, int R, int K, int8_t* codes, void* stream) {
+int apex4_unpack_codes(const void* q_packed, int R, int K, int operand, int8_t* codes, void* stream) {
   if (!codes || !q_packed || R < 1 || K < 1) return APEX4_ERR_INVALID_ARG;
+  if (operand != APEX4_OPERAND_ACT && operand != APEX4_OPERAND_WEIGHT) return APEX4_ERR_INVALID_ARG;
   if (K % kBlockK != 0) return APEX4_ERR_UNSUPPORTED_SHAPE;
   if (!aligned16(codes) || !aligned16(q_packed)) return APEX4_ERR_ALIGNMENT;
   const int a = check_arch();
   if (a != APEX4_OK) return a;
-  return launch_unpack_codes(q_packed, R, K, codes, static_cast<cudaStream_t>(stream)) == cudaSuccess
+  return launch_unpack_codes(q_packed, R, K, codes, operand, static_cast<cudaStream_t>(stream)) == cudaSuccess
              ? APEX4_OK
              : APEX4_ERR_CUDA;
 }
@@ -212,15 +215,11 @@ int apex4_scales_to_natural(const void* s_tiled, int R, int G, void* s_nat, void
 static void fill_params(GemmParams& p, const Dispatch& d, const void* qA, const void* sA,
                         const void* qW, const void* sW, int M, int N, int K, int g) {
   memset(&p, 0, sizeof(p));
-  if (d.swap) {
-    p.qR = static_cast<const uint8_t*>(qW); p.sR = static_cast<const __half*>(sW); p.R = N;
-    p.qC = static_cast<const uint8_t*>(qA); p.sC = static_cast<const __half*>(sA); p.C = M;
-  } else {
-    p.qR = static_cast<const uint8_t*>(qA); p.sR = static_cast<const __half*>(sA); p.R = M;
-    p.qC = static_cast<const uint8_t*>(qW); p.sC = static_cast<const __half*>(sW); p.C = N;
-  }
-  p.K = K; p.g = g; p.G = K / g; p.ldY = N; p.swap = d.swap;
-  p.splits = d.splits; p.kb_per_split = d.kb_per_split;
+  p.qW = static_cast<const uint8_t*>(qW); p.sW = static_cast<const __half*>(sW);
+  p.qA = static_cast<const uint8_t*>(qA); p.sA = static_cast<const __half*>(sA);
+  p.M = M; p.N = N; p.K = K; p.g = g; p.G = K / g;
+  p.tiles_m = d.tiles_m; p.tiles_n = d.tiles_n;
+  p.split = d.split; p.upt = d.upt; p.kbu = d.kbu;
 }
 
 int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
@@ -241,17 +240,15 @@ int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_pa
   GemmParams p;
   fill_params(p, d, qA_packed, sA_f16, qW_packed, sW_f16, M, N, K, g);
   p.Y = Y; p.out_f32 = (out_dtype == APEX4_OUT_F32);
-  if (d.splits > 1) {
-    const size_t need = static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4;
-    const int Rn = d.swap ? N : M, Cn = d.swap ? M : N;
-    const long long tiles = static_cast<long long>((Rn + kTileRows - 1) / kTileRows) * ((Cn + d.nc - 1) / d.nc);
-    if (!workspace || workspace_bytes < need || !aligned16(workspace)) return APEX4_ERR_WORKSPACE;
-    if (tiles > kCounterInts) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  if (d.split) {
+    if (!workspace || workspace_bytes < workspace_need(d, M, N) || !aligned16(workspace))
+      return APEX4_ERR_WORKSPACE;
     p.counters = static_cast<int*>(workspace);
-    p.ws = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + kCounterInts * 4);
+    p.ws = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + counters_bytes(d));
   }
-  return launch_gemm(p, d.nc, false, static_cast<cudaStream_t>(stream)) == cudaSuccess ? APEX4_OK
-                                                                                       : APEX4_ERR_CUDA;
+  return launch_gemm(p, d.nt, d.bias, false, d.grid, static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
 }
 
 int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, int N, int K,
@@ -271,19 +268,23 @@ int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, 
   // packed code buffers are large enough and are only read
   fill_params(p, d, qA_packed, qA_packed, qW_packed, qW_packed, M, N, K, g);
   p.Y = nullptr; p.P_out = P_out; p.pm0 = m0; p.pm1 = m1; p.pn0 = n0; p.pn1 = n1;
-  return launch_gemm(p, d.nc, true, static_cast<cudaStream_t>(stream)) == cudaSuccess ? APEX4_OK
-                                                                                      : APEX4_ERR_CUDA;
+  return launch_gemm(p, d.nt, d.bias, true, d.grid, static_cast<cudaStream_t>(stream)) == cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
 }
 
 static size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+
+static size_t host_ws_bytes(int M, int N, int K, int g) {
+  return align256(workspace_need(choose_dispatch(M, N, K, g), M, N));
+}
 
 size_t apex4_linear_host_scratch_bytes(int M, int N, int K, int group_size, int gran, int layer) {
   if (validate_gemm_shape(M, N, K) != APEX4_OK) return 0;
   const int g = resolve_g(K, group_size, gran, layer);
   if (g < 0) return 0;
-  return align256(static_cast<size_t>(M) * K * 2) + align256(pt4_bytes(M, K)) +
-         align256(st16_elems(M, K / g) * 2) + align256(static_cast<size_t>(M) * N * 4) +
-         align256(static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4);
+  return host_ws_bytes(M, N, K, g) + align256(static_cast<size_t>(M) * K * 2) + align256(pt4_bytes(M, K)) +
+         align256(st16_elems(M, K / g) * 2) + align256(static_cast<size_t>(M) * N * 4);
 }
 
 int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const void* sW_f16,
@@ -299,8 +300,8 @@ int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const 
     return APEX4_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   uint8_t* base = static_cast<uint8_t*>(scratch);
-  uint8_t* ws = base;   // the split-K workspace comes first so that it stays zero-filled across calls
-  const size_t ws_bytes = align256(static_cast<size_t>(kCounterInts) * 4 + static_cast<size_t>(M) * N * 4);
+  uint8_t* ws = base;   // the GEMM workspace comes first so that it stays zero-filled across calls
+  const size_t ws_bytes = host_ws_bytes(M, N, K, g);
   uint8_t* xd = ws + ws_bytes;
   uint8_t* qa = xd + align256(static_cast<size_t>(M) * K * 2);
   uint8_t* sa = qa + align256(pt4_bytes(M, K));
@@ -310,22 +311,22 @@ int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const 
     return APEX4_ERR_CUDA;
   int rc = apex4_quantize_act(xd, M, K, group_size, gran, layer, qa, sa, stream);
   if (rc != APEX4_OK) return rc;
-  rc = apex4_w4a4_gemm(qa, sa, qW_packed, sW_f16, yd, out_dtype, M, N, K, group_size, gran, layer, ws,
-                       ws_bytes, stream);
+  rc = apex4_w4a4_gemm(qa, sa, qW_packed, sW_f16, yd, out_dtype, M, N, K, group_size, gran, layer,
+                       ws_bytes ? ws : nullptr, ws_bytes, stream);
   if (rc != APEX4_OK) return rc;
   if (cudaMemcpyAsync(y_host, yd, ybytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return APEX4_ERR_CUDA;
   return APEX4_OK;
 }
 
-// test hook, not part of the documented ABI: force orientation / tile width / split factor
+// test hooks, not part of the documented ABI: force token-tile width / stream-K / grid size
 // (-1 = automatic).  Process-global; tests restore it.
-int apex4_debug_set_dispatch(int swap, int nc, int splits) {
-  g_force_swap = swap; g_force_nc = nc; g_force_splits = splits;
+int apex4_debug_set_dispatch(int nt, int split, int grid) {
+  g_force_nt = nt; g_force_split = split; g_force_grid = grid;
   return APEX4_OK;
 }
 int apex4_debug_get_dispatch(int M, int N, int K, int g, int* out4) {
   const Dispatch d = choose_dispatch(M, N, K, g);
-  out4[0] = d.swap; out4[1] = d.nc; out4[2] = d.splits; out4[3] = d.kb_per_split;
+  out4[0] = d.nt; out4[1] = d.split; out4[2] = d.grid; out4[3] = d.upt;
   return APEX4_OK;
 }
 

@@ -6,30 +6,30 @@
 
 namespace apex4 {
 
-// The kernel works on two abstract operands, both in PT4/ST16 layout:
-//   "R side" = tcgen05 A operand: 128-row tiles -> TMEM lanes (one epilogue thread per row)
-//   "C side" = tcgen05 B operand: NC-row tiles  -> TMEM columns
-// Normal orientation (swap = 0): R = activations (rows m), C = weights (rows n), Y[r, c].
-// Swapped (swap = 1, decode-sized M): R = weights (rows n), C = activations (rows m), Y[c, r].
+// The kernel always runs "weights on the TMEM lanes": a work tile is 128 weight rows (n) x NT token
+// rows (m), NT in {16, 32, 64, 128, 256}.  Weights (PW4/ST16) are the tcgen05 A operand (widened in
+// registers, stored to TMEM); activations (PT4/ST16) are the B operand (widened in shared memory).
 struct GemmParams {
-  const uint8_t* qR;
-  const __half* sR;
-  const uint8_t* qC;
-  const __half* sC;
-  void* Y;
+  const uint8_t* qW;   // PW4  [Np/128][K/128][8192]
+  const __half* sW;    // ST16 [Np/128][G][128]
+  const uint8_t* qA;   // PT4  [Mp/128][K/128][8192]
+  const __half* sA;    // ST16 [Mp/128][G][128]
+  void* Y;             // [M, N] row-major, FP16 or FP32; nullptr for the debug dump
   int out_f32;
-  int R, C;        // logical row counts of the two operands
-  int K, g, G;
-  int ldY;         // N (row pitch of Y in elements)
-  int swap;
-  int splits;      // split-K factor (grid.z); 1 = direct store
-  int kb_per_split;
-  float* ws;       // split-K: FP32 partial sums [M, N], zero on entry, zero on exit
-  int* counters;   // split-K: one arrival counter per (r tile, c tile), zero on entry/exit
-  int32_t* P_out;  // debug dump of per-group INT32 sums (DUMP kernels only)
+  int M, N, K, g, G;
+  int tiles_m, tiles_n;   // ceil(M / NT), ceil(N / 128)
+  // work distribution (a6 / PAPER.md:226-230): split = 0 -> CTA c owns whole tiles c, c + grid, ...;
+  // split = 1 -> the K loop of all tiles is one line of `units` dealt to the CTAs in equal contiguous
+  // ranges (stream-K); a unit is kbu k-blocks (one group when g >= 128), a tile has upt units.
+  int split, upt, kbu;
+  float* ws;           // split = 1: FP32 partial sums [M, N], zero on entry, zero on exit
+  int* counters;       // split = 1: finished units per tile, zero on entry/exit
+  int32_t* P_out;      // debug dump of the per-group INT32 sums (DUMP kernels only)
   int pm0, pm1, pn0, pn1;
 };
 
-cudaError_t launch_gemm(const GemmParams& p, int nc, bool dump, cudaStream_t st);
+// nt: token-tile width (16/32/64/128/256); bias: magic-biased accumulators (g <= 128) or I2F (g >= 256)
+cudaError_t launch_gemm(const GemmParams& p, int nt, bool bias, bool dump, int grid, cudaStream_t st);
+int gemm_max_ctas();   // persistent grid size: one CTA per SM
 
 }  // namespace apex4

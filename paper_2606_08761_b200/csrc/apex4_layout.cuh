@@ -13,6 +13,13 @@
 //       code(rr, kb*128 + p) lives in blob byte  rr*64 + j*16 + y,  nibble h (0 = low, 1 = high).
 //   (Any order inside a K=32 slice would give the same integer sums; identity keeps g=32 simple.)
 //
+// PW4 (packed INT4 weight codes).  Same blobs, same sizes.  The GEMM's widener thread r reads its own
+//   64-byte row, widens it in registers and stores the 32 INT8 words to TMEM, where the tensor core
+//   reads the A operand as: 32-bit column c of lane r = k bytes 4c..4c+3 of the k-block.  Logical
+//   chunk j (= the K=32 slice j of the k-block) holds element k = kb*128 + 32j + p in byte p & 15,
+//   nibble p >> 4.  Only the 16-byte chunk SLOT is permuted, slot = j ^ ((rr >> 1) & 3), so that the
+//   128-bit loads of eight consecutive rows cover all 32 banks.
+//
 // ST16 (FP16 scales).  [Rp/128][G][128]: element (r, gamma) at ((r/128)*G + gamma)*128 + r%128, so
 //   the scales of one 128-row tile for consecutive groups are one contiguous bulk copy.
 #pragma once

@@ -1,5 +1,5 @@
 // apex4_quant.cu -- a0/a1 of the hot path: the symmetric INT4 group quantizer of Eq. 7
-// (PAPER.md:146-150), used online for activations and offline for weights, writing the PT4 / ST16
+// (PAPER.md:146-150), used online for activations and offline for weights, writing the PT4 / PW4 / ST16
 // device layouts of apex4_layout.cuh; plus the code packer / unpacker and scale re-layout twins.
 //
 // Arithmetic (readings R1-R5 of DESIGN.md): a = max|x| exact in FP16; S = fp16_rn(float(a) / 7.0f)
@@ -27,8 +27,9 @@ __device__ __forceinline__ int quant_one(float x, float s) {
   return max(-8, min(7, q));
 }
 
-// 32 FP16 values (4 x uint4) -> 16 packed bytes (one PT4 chunk) for blob row rr.
-__device__ __forceinline__ uint4 quant_pack_chunk(const uint4 (&v)[4], float s, int rr) {
+// 32 FP16 values (4 x uint4) -> 16 packed bytes (one PT4 / PW4 chunk).  swap: the second
+// 16-element half lands in the low nibbles (PT4 odd rows; never for PW4, apex4_layout.cuh).
+__device__ __forceinline__ uint4 quant_pack_chunk(const uint4 (&v)[4], float s, int swap) {
   int code[32];
   const uint32_t* w = reinterpret_cast<const uint32_t*>(v);
 #pragma unroll
@@ -38,7 +39,6 @@ __device__ __forceinline__ uint4 quant_pack_chunk(const uint4 (&v)[4], float s, 
     code[2 * i] = (s == 0.f) ? 0 : quant_one(f.x, s);
     code[2 * i + 1] = (s == 0.f) ? 0 : quant_one(f.y, s);
   }
-  const int swap = rr & 1;   // which 16-element half lands in the low nibbles (apex4_layout.cuh)
   uint32_t out[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -74,7 +74,7 @@ __device__ __forceinline__ size_t chunk_dst_offset(int r, int c, int K) {
 template <int GL>
 __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __restrict__ X, int R,
                                                                int K, uint8_t* __restrict__ q,
-                                                               __half* __restrict__ S) {
+                                                               __half* __restrict__ S, int weights) {
   const int cpr = K / 32;
   const long long total = static_cast<long long>(R) * cpr;
   long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __r
   }
   __half Sh;
   const float s = scale_from_absmax_bits(m, &Sh);
-  const uint4 packed = quant_pack_chunk(v, s, r % kTileRows);
+  const uint4 packed = quant_pack_chunk(v, s, weights ? 0 : (r & 1));
   if (active) {
     *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c, K)) = packed;
     if ((c % GL) == 0) S[st16_index(r, c / GL, cpr / GL)] = Sh;
@@ -117,7 +117,7 @@ constexpr int kLargeThreads = 256;
 constexpr int kLargeUnroll = 4;
 __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
     const __half* __restrict__ X, int R, int K, int g, uint8_t* __restrict__ q,
-    __half* __restrict__ S) {
+    __half* __restrict__ S, int weights) {
   const int G = K / g;
   const int r = blockIdx.x / G;
   const int gamma = blockIdx.x % G;
@@ -163,15 +163,15 @@ __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
   for (int u = 0; u < kLargeUnroll; ++u) {
     const int cl = threadIdx.x + u * kLargeThreads;
     if (cl < cpg) {
-      const uint4 packed = quant_pack_chunk(v[u], s, r % kTileRows);
+      const uint4 packed = quant_pack_chunk(v[u], s, weights ? 0 : (r & 1));
       *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c0 + cl, K)) = packed;
     }
   }
 }
 
-// codes int8 [R,K] -> PT4
+// codes int8 [R,K] -> PT4 (weights = 0) / PW4 (weights = 1)
 __global__ void __launch_bounds__(256) pack_codes_kernel(const int8_t* __restrict__ codes, int R,
-                                                         int K, uint8_t* __restrict__ q) {
+                                                         int K, uint8_t* __restrict__ q, int weights) {
   const int cpr = K / 32;
   const long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (gid >= static_cast<long long>(R) * cpr) return;
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256) pack_codes_kernel(const int8_t* __restric
   const uint4* src = reinterpret_cast<const uint4*>(codes + static_cast<size_t>(r) * K + c * 32);
   uint4 in[2] = {__ldg(src), __ldg(src + 1)};
   const int8_t* cd = reinterpret_cast<const int8_t*>(in);
-  const int swap = r & 1;
+  const int swap = weights ? 0 : (r & 1);
   uint32_t out[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -196,16 +196,16 @@ __global__ void __launch_bounds__(256) pack_codes_kernel(const int8_t* __restric
   *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c, K)) = make_uint4(out[0], out[1], out[2], out[3]);
 }
 
-// PT4 -> codes int8 [R,K]
+// PT4 / PW4 -> codes int8 [R,K]
 __global__ void __launch_bounds__(256) unpack_codes_kernel(const uint8_t* __restrict__ q, int R,
-                                                           int K, int8_t* __restrict__ codes) {
+                                                           int K, int8_t* __restrict__ codes, int weights) {
   const int cpr = K / 32;
   const long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (gid >= static_cast<long long>(R) * cpr) return;
   const int r = static_cast<int>(gid / cpr), c = static_cast<int>(gid % cpr);
   const uint4 p = __ldg(reinterpret_cast<const uint4*>(q + chunk_dst_offset(r, c, K)));
   const uint8_t* pb = reinterpret_cast<const uint8_t*>(&p);
-  const int swap = r & 1;
+  const int swap = weights ? 0 : (r & 1);
   int8_t out[32];
 #pragma unroll
   for (int y = 0; y < 16; ++y) {
@@ -241,7 +241,8 @@ __global__ void scales_to_natural_kernel(const __half* __restrict__ tiled, int R
 }
 
 // ---------------------------------------------------------------------------------- launchers
-cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, cudaStream_t st) {
+cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, int weights,
+                            cudaStream_t st) {
   const __half* X = static_cast<const __half*>(x);
   uint8_t* Q = static_cast<uint8_t*>(q);
   __half* S = static_cast<__half*>(s);
@@ -251,17 +252,17 @@ cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s
   const bool pow2 = (gl & (gl - 1)) == 0;
   if (pow2 && gl <= 32) {
     switch (gl) {
-      case 1: quantize_small_g_kernel<1><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
-      case 2: quantize_small_g_kernel<2><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
-      case 4: quantize_small_g_kernel<4><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
-      case 8: quantize_small_g_kernel<8><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
-      case 16: quantize_small_g_kernel<16><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
-      default: quantize_small_g_kernel<32><<<blocks, 256, 0, st>>>(X, R, K, Q, S); break;
+      case 1: quantize_small_g_kernel<1><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
+      case 2: quantize_small_g_kernel<2><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
+      case 4: quantize_small_g_kernel<4><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
+      case 8: quantize_small_g_kernel<8><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
+      case 16: quantize_small_g_kernel<16><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
+      default: quantize_small_g_kernel<32><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
     }
   } else {
     if (gl > kLargeThreads * kLargeUnroll) return cudaErrorInvalidValue;
     const long long nb = static_cast<long long>(R) * (K / g);
-    quantize_large_g_kernel<<<static_cast<unsigned>(nb), kLargeThreads, 0, st>>>(X, R, K, g, Q, S);
+    quantize_large_g_kernel<<<static_cast<unsigned>(nb), kLargeThreads, 0, st>>>(X, R, K, g, Q, S, weights);
   }
   return cudaGetLastError();
 }
@@ -269,16 +270,16 @@ bool quantize_supports_group(int g) {
   const int gl = g / 32;
   return ((gl & (gl - 1)) == 0 && gl <= 32) || gl <= kLargeThreads * kLargeUnroll;
 }
-cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, cudaStream_t st) {
+cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, int weights, cudaStream_t st) {
   const long long total = static_cast<long long>(R) * (K / 32);
   pack_codes_kernel<<<static_cast<unsigned>((total + 255) / 256), 256, 0, st>>>(
-      codes, R, K, static_cast<uint8_t*>(q));
+      codes, R, K, static_cast<uint8_t*>(q), weights);
   return cudaGetLastError();
 }
-cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, cudaStream_t st) {
+cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, int weights, cudaStream_t st) {
   const long long total = static_cast<long long>(R) * (K / 32);
   unpack_codes_kernel<<<static_cast<unsigned>((total + 255) / 256), 256, 0, st>>>(
-      static_cast<const uint8_t*>(q), R, K, codes);
+      static_cast<const uint8_t*>(q), R, K, codes, weights);
   return cudaGetLastError();
 }
 cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st) {

@@ -75,13 +75,15 @@ def test_argument_validation_without_gpu(L):
 
 
 def test_dispatch_table(L):
+    """Host-side choice of token-tile width / work distribution (a6, a8): pure host code."""
     from paper_2606_08761_b200 import apex4
-    swap, nc, splits, kbps = apex4.debug_get_dispatch(16, 8192, 8192, 128)
-    assert swap == 1 and nc == 16 and splits >= 2 and kbps * splits >= 64
-    swap, nc, splits, kbps = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
-    assert (swap, nc, splits, kbps) == (0, 256, 1, 64)
+    nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 128)
+    assert (nt, split, upt) == (16, 1, 64) and 1 <= grid <= 148     # decode: stream-K over all SMs
+    nt, split, grid, upt = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
+    assert (nt, split, upt) == (256, 0, 64)                          # 2048 tiles: whole tiles per CTA
     # per-channel: the k range cannot be split inside a group
-    swap, nc, splits, kbps = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
-    assert splits == 1 and kbps == 64
+    nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
+    assert (nt, split, grid, upt) == (16, 0, 64, 1)
     assert apex4.workspace_bytes(8192, 8192, 8192, 128) == 0
-    assert apex4.workspace_bytes(16, 8192, 8192, 128) == 4096 * 4 + 16 * 8192 * 4
+    assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0
+    assert apex4.workspace_bytes(16, 8192, 8192, 128) == 256 + 16 * 8192 * 4

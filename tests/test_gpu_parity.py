@@ -30,7 +30,7 @@ def gpu_quantize(A, X, g, weights=False):
     fn = A.pack_weights if weights else A.quantize_act
     q, s, g_res = fn(dev(X), g)
     assert g_res == g
-    codes = A.unpack_codes(q, R, K).cpu().numpy()
+    codes = A.unpack_codes(q, R, K, A.OPERAND_WEIGHT if weights else A.OPERAND_ACT).cpu().numpy()
     scales = A.scales_to_natural(s, R, K // g).cpu().numpy()
     return q, s, codes, scales
 
@@ -98,9 +98,10 @@ def test_quantizer_exhaustive_fp16_inputs(A):
 def test_pack_unpack_roundtrip_and_scale_layout(A):
     rng = np.random.default_rng(9)
     codes = rng.integers(-8, 8, size=(200, 640)).astype(np.int8)
-    q = A.pack_codes(dev(codes))
-    assert q.numel() == A.packed_bytes(200, 640)
-    assert np.array_equal(A.unpack_codes(q, 200, 640).cpu().numpy(), codes)
+    for operand in (A.OPERAND_ACT, A.OPERAND_WEIGHT):
+        q = A.pack_codes(dev(codes), operand)
+        assert q.numel() == A.packed_bytes(200, 640)
+        assert np.array_equal(A.unpack_codes(q, 200, 640, operand).cpu().numpy(), codes)
     s = rng.standard_normal((200, 5)).astype(np.float16)
     t = A.scales_from_natural(dev(s))
     assert np.array_equal(A.scales_to_natural(t, 200, 5).cpu().numpy().view(np.uint16), s.view(np.uint16))
@@ -147,10 +148,11 @@ def test_gemm_config0(A):
 
 
 @pytest.mark.parametrize("g", [32, 64, 128, 256, 512])
-@pytest.mark.parametrize("dispatch", [(0, 128, 1), (0, 256, 1), (1, 16, 1), (1, 16, 2), (0, 128, 2),
-                                      (1, 64, 1), (1, 32, 4)])
+@pytest.mark.parametrize("dispatch", [(16, 0, -1), (16, 1, -1), (16, 1, 3), (32, 0, -1), (32, 1, 5),
+                                      (64, 1, -1), (128, 0, 1), (128, 1, 7), (256, 0, -1), (256, 1, 3)])
 def test_gemm_config0_all_dispatches(A, g, dispatch):
-    """Same problem through both orientations, several tile widths and split-K factors."""
+    """Same problem through every token-tile width, whole-tile and stream-K work distribution and
+    several grid sizes (dispatch = (tile width, stream-K, CTAs))."""
     run_gemm_case(A, 16, 256, 512, g, seed=0, fixed=True, dispatch=dispatch)
 
 
@@ -186,7 +188,7 @@ def test_gemm_minus8_codes_headroom(A):
     M, N, K = 8, 128, 4096
     cA = np.full((M, K), -8, dtype=np.int8)
     cW = np.full((N, K), -8, dtype=np.int8)
-    qA, qW = A.pack_codes(dev(cA)), A.pack_codes(dev(cW))
+    qA, qW = A.pack_codes(dev(cA), A.OPERAND_ACT), A.pack_codes(dev(cW), A.OPERAND_WEIGHT)
     for g in (32, 128, K):
         P = A.debug_group_sums(qA, qW, M, N, K, g).cpu().numpy()
         assert np.all(P == 64 * g)
@@ -236,8 +238,8 @@ def test_error_codes_on_device(A):
         A.quantize_act(x, 48)
     assert e.value.status == A.ERR_UNSUPPORTED_SHAPE
     q, s, _ = A.quantize_act(x, 128)
-    with pytest.raises(A.Apex4Error) as e:     # split-K dispatch without a workspace
-        A.lib().apex4_debug_set_dispatch(1, 16, 2)
+    with pytest.raises(A.Apex4Error) as e:     # stream-K dispatch without a workspace
+        A.lib().apex4_debug_set_dispatch(16, 1, 2)
         try:
             st = A.lib().apex4_w4a4_gemm(q.data_ptr(), s.data_ptr(), q.data_ptr(), s.data_ptr(), x.data_ptr(),
                                          0, 16, 128, 512, 128, 0, 0, None, 0, None)
