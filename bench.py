@@ -51,44 +51,56 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region: the sampler is started
+    before the warm-up (nvidia-smi takes a few hundred ms to come up), every row is stamped with the
+    host clock when it is read, and stop(t0, t1) keeps the rows that fall inside the timed window."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index=0):
-        self.index, self.rows, self.proc = index, [], None
+    def __init__(self, index=0, period_ms=20):
+        self.index, self.rows, self.proc, self.period_ms = index, [], None, period_ms
 
-    def start(self):
+    def start(self, wait_s=5.0):
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", str(self.period_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
             self.proc = None
+            return
+        t_end = time.time() + wait_s
+        while not self.rows and time.time() < t_end:
+            time.sleep(0.01)
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(2.5 * self.period_ms * 1e-3)
         self.proc.terminate()
         self.t.join(timeout=2)
-        sm, mx, reasons = [], None, set()
-        for r in self.rows:
+        rows = [r for (ts, r) in self.rows if (t0 is None or ts >= t0) and (t1 is None or ts <= t1 + 2e-3 * self.period_ms)]
+        window = "timed region"
+        if not rows:                      # region shorter than one sampling period: nearest rows after its start
+            rows = [r for (ts, r) in self.rows if t0 is None or ts >= t0][:3] or [r for (_, r) in self.rows[-3:]]
+            window = "nearest samples (timed region shorter than the sampling period)"
+        sm, mx, pw, reasons = [], None, [], set()
+        for r in rows:
             try:
-                sm.append(float(r[0])); mx = float(r[1])
+                sm.append(float(r[0])); mx = float(r[1]); pw.append(float(r[2]))
             except (ValueError, IndexError):
                 continue
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "window": window}
 
 
 def oracle_sample(sample_rows):
@@ -141,8 +153,8 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="apex4")
     ap.add_argument("--sweep", action="store_true", help="also time the config-2 M sweep + cuBLAS FP16")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -218,13 +230,15 @@ def main():
             ms = float(t.item())
         return ms
 
-    for _ in range(args.warmup):
-        step()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for _ in range(args.warmup):
+        step()
+    t0 = time.time()
     ms = timed(step, args.steps)
-    clocks = sampler.stop() if rank == 0 else None
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
     ops = total_ops(ls)
     value = world * ops * args.steps / (ms * 1e-3) * 1e-12
 
