@@ -61,7 +61,7 @@ int resolve_g(int K, int group_size, int gran, int layer) {
 }
 
 struct Dispatch {
-  int nt;      // token-tile width
+  int nt;      // token-tile width; 256 = CTA-pair kernel (256 x 256 tiles, grid counted in pairs)
   int bias;    // magic-biased accumulators (g <= 128)
   int split;   // stream-K work distribution (needs the workspace)
   int grid;
@@ -83,11 +83,13 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
   else if (M <= 64) d.nt = 64;
   else if (M <= 128) d.nt = 128;
   else d.nt = 256;
+  const bool pair = d.nt == 256;
   d.tiles_m = (M + d.nt - 1) / d.nt;
-  d.tiles_n = (N + kTileRows - 1) / kTileRows;
+  d.tiles_n = pair ? (N + 2 * kTileRows - 1) / (2 * kTileRows) : (N + kTileRows - 1) / kTileRows;
   const long long tiles = static_cast<long long>(d.tiles_m) * d.tiles_n;
   const long long units = tiles * d.upt;
-  const int sms = g_force_grid > 0 ? g_force_grid : gemm_max_ctas();
+  const int max_grid = pair ? gemm_max_pairs() : gemm_max_ctas();
+  const int sms = (g_force_grid > 0 && g_force_grid < max_grid) ? g_force_grid : max_grid;
   d.grid = static_cast<int>(units < sms ? units : sms);
   // whole tiles per CTA when the last wave is reasonably full, stream-K otherwise
   const long long waves = (tiles + d.grid - 1) / d.grid;
@@ -99,7 +101,12 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
 }
 
 size_t counters_bytes(const Dispatch& d) {
-  return (static_cast<size_t>(d.tiles_m) * d.tiles_n * 4 + 255) / 256 * 256;
+  return (static_cast<size_t>(d.tiles_m) * d.tiles_n * (d.nt == 256 ? 2 : 1) * 4 + 255) / 256 * 256;
+}
+
+cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
+  if (d.nt == 256) return launch_gemm_pair(p, d.bias, dump, d.grid, st);
+  return launch_gemm(p, d.nt, d.bias, dump, d.grid, st);
 }
 size_t workspace_need(const Dispatch& d, int M, int N) {
   return d.split ? counters_bytes(d) + static_cast<size_t>(M) * N * 4 : 0;
@@ -246,7 +253,7 @@ int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_pa
     p.counters = static_cast<int*>(workspace);
     p.ws = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + counters_bytes(d));
   }
-  return launch_gemm(p, d.nt, d.bias, false, d.grid, static_cast<cudaStream_t>(stream)) == cudaSuccess
+  return launch_dispatch(p, d, false, static_cast<cudaStream_t>(stream)) == cudaSuccess
              ? APEX4_OK
              : APEX4_ERR_CUDA;
 }
@@ -268,7 +275,7 @@ int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, 
   // packed code buffers are large enough and are only read
   fill_params(p, d, qA_packed, qA_packed, qW_packed, qW_packed, M, N, K, g);
   p.Y = nullptr; p.P_out = P_out; p.pm0 = m0; p.pm1 = m1; p.pn0 = n0; p.pn1 = n1;
-  return launch_gemm(p, d.nt, d.bias, true, d.grid, static_cast<cudaStream_t>(stream)) == cudaSuccess
+  return launch_dispatch(p, d, true, static_cast<cudaStream_t>(stream)) == cudaSuccess
              ? APEX4_OK
              : APEX4_ERR_CUDA;
 }

@@ -511,7 +511,6 @@ cudaError_t launch_gemm(const GemmParams& p, int nt, bool bias, bool dump, int g
     case 32: return launch_nt<32>(p, bias, dump, grid, st);
     case 64: return launch_nt<64>(p, bias, dump, grid, st);
     case 128: return launch_nt<128>(p, bias, dump, grid, st);
-    case 256: return launch_nt<256>(p, bias, dump, grid, st);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -32,4 +32,10 @@ struct GemmParams {
 cudaError_t launch_gemm(const GemmParams& p, int nt, bool bias, bool dump, int grid, cudaStream_t st);
 int gemm_max_ctas();   // persistent grid size: one CTA per SM
 
+// Tensor-bound regime (apex4_gemm_pair.cu): CTA pairs (cluster of 2, cta_group::2), work tile = 256
+// weight rows x 256 tokens; tiles_m / tiles_n / counters are in units of pair tiles (counters: two per
+// tile, one per CTA of the pair).  npairs <= gemm_max_pairs().
+cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st);
+int gemm_max_pairs();
+
 }  // namespace apex4
