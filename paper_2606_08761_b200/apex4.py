@@ -14,7 +14,7 @@ from typing import Optional, Tuple
 import torch
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_PKG, "libapex4.so")
+LIB_PATH = os.environ.get("APEX4_LIB") or os.path.join(_PKG, "libapex4.so")   # APEX4_LIB: load another build
 
 # enums of include/apex4.h
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_SHAPE, ERR_ALIGNMENT, ERR_WORKSPACE, ERR_CUDA, ERR_ARCH = range(7)
@@ -80,6 +80,7 @@ def lib() -> ctypes.CDLL:
     L.apex4_debug_group_sums.argtypes = [c_void_p, c_void_p] + [c_int] * 10 + [c_void_p, c_void_p]
     L.apex4_measure_rho.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
     L.apex4_debug_set_dispatch.argtypes = [c_int, c_int, c_int]
+    L.apex4_debug_set_timeline.argtypes = [c_void_p]
     L.apex4_debug_get_dispatch.argtypes = [c_int, c_int, c_int, c_int, ctypes.POINTER(c_int)]
     for name in ("apex4_pack_codes", "apex4_unpack_codes", "apex4_scales_from_natural",
                  "apex4_scales_to_natural", "apex4_w4a4_gemm", "apex4_w4a4_linear_host",

@@ -2,6 +2,8 @@
 // choice of token-tile width and work distribution (whole tiles / stream-K) for the GEMM kernel.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "../../include/apex4.h"
@@ -70,6 +72,7 @@ struct Dispatch {
 
 // test hook (apex4_debug_set_dispatch): -1 = automatic
 int g_force_nt = -1, g_force_split = -1, g_force_grid = -1;
+long long* g_timeline = nullptr;
 
 Dispatch choose_dispatch(int M, int N, int K, int g) {
   Dispatch d;
@@ -84,7 +87,7 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
   else if (M <= 128) d.nt = 128;
   else d.nt = 256;
   const bool pair = d.nt == 256;
-  d.tiles_m = (M + d.nt - 1) / d.nt;
+  d.tiles_m = pair ? (M + kPairTokens - 1) / kPairTokens : (M + d.nt - 1) / d.nt;
   d.tiles_n = pair ? (N + 2 * kTileRows - 1) / (2 * kTileRows) : (N + kTileRows - 1) / kTileRows;
   const long long tiles = static_cast<long long>(d.tiles_m) * d.tiles_n;
   const long long units = tiles * d.upt;
@@ -105,8 +108,11 @@ size_t counters_bytes(const Dispatch& d) {
 }
 
 cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
-  if (d.nt == 256) return launch_gemm_pair(p, d.bias, dump, d.grid, st);
-  return launch_gemm(p, d.nt, d.bias, dump, d.grid, st);
+  const cudaError_t e = d.nt == 256 ? launch_gemm_pair(p, d.bias, dump, d.grid, st)
+                                    : launch_gemm(p, d.nt, d.bias, dump, d.grid, st);
+  if (e != cudaSuccess && getenv("APEX4_VERBOSE"))
+    fprintf(stderr, "apex4: GEMM launch (tile %d, grid %d) failed: %s\n", d.nt, d.grid, cudaGetErrorString(e));
+  return e;
 }
 size_t workspace_need(const Dispatch& d, int M, int N) {
   return d.split ? counters_bytes(d) + static_cast<size_t>(M) * N * 4 : 0;
@@ -227,6 +233,7 @@ static void fill_params(GemmParams& p, const Dispatch& d, const void* qA, const 
   p.M = M; p.N = N; p.K = K; p.g = g; p.G = K / g;
   p.tiles_m = d.tiles_m; p.tiles_n = d.tiles_n;
   p.split = d.split; p.upt = d.upt; p.kbu = d.kbu;
+  p.tl = g_timeline;
 }
 
 int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
@@ -329,6 +336,10 @@ int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const 
 // (-1 = automatic).  Process-global; tests restore it.
 int apex4_debug_set_dispatch(int nt, int split, int grid) {
   g_force_nt = nt; g_force_split = split; g_force_grid = grid;
+  return APEX4_OK;
+}
+int apex4_debug_set_timeline(void* dev_buf) {
+  g_timeline = static_cast<long long*>(dev_buf);
   return APEX4_OK;
 }
 int apex4_debug_get_dispatch(int M, int N, int K, int g, int* out4) {

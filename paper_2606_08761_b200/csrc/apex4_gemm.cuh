@@ -26,14 +26,17 @@ struct GemmParams {
   int* counters;       // split = 1: finished units per tile, zero on entry/exit
   int32_t* P_out;      // debug dump of the per-group INT32 sums (DUMP kernels only)
   int pm0, pm1, pn0, pn1;
+  long long* tl;       // debug timeline (test hook): clock64 stamps of CTA 0, [event][64 k-blocks]; normally null
 };
 
 // nt: token-tile width (16/32/64/128/256); bias: magic-biased accumulators (g <= 128) or I2F (g >= 256)
 cudaError_t launch_gemm(const GemmParams& p, int nt, bool bias, bool dump, int grid, cudaStream_t st);
 int gemm_max_ctas();   // persistent grid size: one CTA per SM
 
+constexpr int kPairTokens = 192;   // tokens per CTA-pair tile
+
 // Tensor-bound regime (apex4_gemm_pair.cu): CTA pairs (cluster of 2, cta_group::2), work tile = 256
-// weight rows x 256 tokens; tiles_m / tiles_n / counters are in units of pair tiles (counters: two per
+// weight rows x kPairTokens tokens; tiles_m / tiles_n / counters are in units of pair tiles (counters: two per
 // tile, one per CTA of the pair).  npairs <= gemm_max_pairs().
 cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st);
 int gemm_max_pairs();

@@ -1,30 +1,35 @@
 // apex4_gemm_pair.cu -- a2..a7 of the hot path for the tensor-bound regime (M > 128): the W4A4
 // group-dequant GEMM of Eq. 8 on a CTA PAIR (cluster of 2, tcgen05 cta_group::2).
 //
-// A pair owns a 256 (weight rows n) x 256 (tokens m) output tile.  CTA r of the pair holds weight
-// rows 128 r .. 128 r + 127 of the tile on its 128 TMEM lanes and supplies one half of the token
-// rows of every MMA from its own shared memory, so per SM and k-block (K = 128) only 8 KB of packed
-// weights and 8 KB of packed activations are fetched, widened and read by the tensor core: half the
-// L2 traffic, half the activation widening and half the shared-memory operand reads of a lone CTA
+// A pair owns a 256 (weight rows n) x 192 (tokens m) output tile.  CTA r of the pair holds weight
+// rows 128 r .. 128 r + 127 of the tile on its 128 TMEM lanes and supplies 96 of the 192 token rows
+// of every MMA from its own shared memory, so per SM and k-block (K = 128) only 8 KB of packed
+// weights and 6 KB of packed activations are fetched, widened and read by the tensor core
 // (shared-memory read bandwidth is the scarce resource, profiles/r1_ubench_b200.md).
 //
-// Roles (512 threads per CTA):
-//   warp 0      producer : 1-D bulk async copies (UBLKCP) of this CTA's packed INT4 rows + FP16 scales
-//   warp 1      MMA      : leader CTA only; tcgen05.mma cta_group::2 kind::i8, M = 256, N = 128, K = 32,
-//                          A (weights) from TMEM, B (tokens) from shared memory, three half-tile
-//                          accumulator buffers of 128 columns; tcgen05.commit multicast to both CTAs
-//   warps 4-7   wideners : INT4 -> INT8 (x16).  Thread r widens weight row r in registers and stores it
-//                          to TMEM; 128 token rows are widened smem -> smem into the 128B-swizzled
-//                          UMMA layout.  One elected arrive per warp on the LEADER's operand barrier.
-//                          Also FP16 -> FP32 scale preparation.
-//   warps 8-15  epilogue : warpgroup h owns the tokens of half h.  tcgen05.ld in the 16x256b shape
+// Why 192 tokens: (1) TMEM holds two full 192-column accumulator buffers plus four 32-column
+// weight-operand stages (2 x 192 + 4 x 32 = 512), so the MMA of group g+1 runs while the epilogue
+// drains group g; (2) an epilogue thread keeps 96 FP32 running sums, which leaves registers for a
+// true software prefetch of the next TMEM chunk (with 128 sums ptxas serialised load and arithmetic).
+//
+// Roles (640 threads per CTA; launched with 96 registers per thread = the 61 440-register pool that
+// setmaxnreg then redistributes: control 32, wideners 40, epilogue 184):
+//   warps 0-7   wideners : two warpgroups, k-blocks dealt alternately.  INT4 -> INT8 (x16).  Thread r
+//                          widens weight row r in registers and stores it to TMEM; 96 token rows are
+//                          widened smem -> smem into the 128B-swizzled UMMA layout.  One elected
+//                          arrive per warp on the LEADER's operand barrier.  FP16 -> FP32 scale prep.
+//   warps 8-15  epilogue : warpgroup h owns tokens 96 h .. 96 h + 95.  tcgen05.ld in the 16x256b shape
 //                          (thread = 4 rows x 4 columns of a 16-column chunk, so one LDS.128 fetches
-//                          the four token scales a chunk needs instead of sixteen), chunk c+1 is
-//                          loaded while chunk c is in the FMA pipe and the buffer goes back to the
-//                          MMA warp before the last chunk's arithmetic.  Two FFMA2 per element pair:
-//                          fma(f, sW/256, -49152 sW) = P sW rounded once (magic-biased accumulators,
-//                          see apex4_gemm.cu), then fma with sA into the FP32 running sums.
-#include <cooperative_groups.h>
+//                          the four token scales a chunk needs), chunk c+1 in flight while chunk c is
+//                          in the FMA pipe.  Two FFMA2 per element pair: fma(f, sW/256, -49152 sW) =
+//                          P sW rounded once (magic-biased accumulators, see apex4_gemm.cu), then fma
+//                          with sA into the FP32 running sums.
+//   warp 16     producer : 1-D bulk async copies (UBLKCP) of this CTA's packed INT4 rows + FP16 scales
+//   warp 17     MMA      : leader CTA only; tcgen05.mma cta_group::2 kind::i8, M = 256, N = 192, K = 32,
+//                          A (weights) from TMEM, B (tokens) from shared memory; tcgen05.commit
+//                          multicast to both CTAs.  Producer and MMA loops run warp-uniform with one
+//                          elected lane issuing (operands in uniform registers, no divisions).
+#include <type_traits>
 
 #include "apex4_gemm.cuh"
 #include "apex4_layout.cuh"
@@ -35,31 +40,38 @@ namespace apex4 {
 namespace pair {
 
 constexpr uint32_t kMagicBits = 0x4B400000u;   // float 12582912 = 1.5 * 2^23
-constexpr int kThreads = 512;
-constexpr int kNT = 256;            // tokens per pair tile
-constexpr int kNB = 128;            // tokens per half = MMA N = accumulator buffer width
-constexpr int kAccBufs = 3;
+constexpr int kWidenWGs = 2;        // widener warpgroups (k-blocks dealt alternately)
+constexpr int kEpiWarp0 = 4 * kWidenWGs;       // first epilogue warp
+constexpr int kCtlWarp0 = kEpiWarp0 + 8;       // producer warp; the MMA warp follows
+constexpr int kThreads = 32 * (kCtlWarp0 + 4); // warps are allocated in fours: two control warps idle
+constexpr int kNT = kPairTokens;    // 192 tokens per pair tile = MMA N = accumulator buffer width
+constexpr int kHalf = kNT / 2;      // 96 token rows per CTA / columns per epilogue warpgroup
+constexpr int kChunks = kHalf / 16; // 16-column TMEM chunks per epilogue thread
+constexpr int kAccBufs = 2;
 constexpr int kOpStages = 4;        // widened operand stages (TMEM A + smem B)
-constexpr int kPkStages = 5;        // packed (bulk copy) stages
+constexpr int kPkStages = 6;        // packed (bulk copy) stages
 constexpr int kScfSlots = 8;
 constexpr int kTmemA0 = 384;        // first TMEM column of the A-operand stages
 constexpr int kPkWBytes = kBlobBytes;             // 128 weight rows of a k-block
-constexpr int kPkABytes = 2 * 64 * kRowBytes;     // 64 token rows of each half
+constexpr int kPkABytes = kHalf * kRowBytes;      // 96 token rows
 constexpr int kPkSWBytes = 4 * 256;               // up to 4 groups per k-block, 128 FP16 each
-constexpr int kPkSABytes = 2 * 4 * 256;           // two 128-token blobs
+constexpr int kPkSABytes = 2 * 4 * 256;           // the two 128-token blobs the tile touches
 constexpr int kPkStageBytes = kPkWBytes + kPkABytes + kPkSWBytes + kPkSABytes;
-constexpr int kI8StageBytes = 128 * kBlockK;      // widened tokens: [half][64 rows][128 B]
-constexpr int kScfSlotBytes = kTileRows * 8 + kNT * 4;
-constexpr int kRegsCtl = 32, kRegsWiden = 64, kRegsEpi = 208;
+constexpr int kI8StageBytes = kHalf * kBlockK;    // widened tokens: [96 rows][128 B]
+constexpr int kScfSlotBytes = kTileRows * 8 + kNT * 4 + 256;   // {a,b} per row, sA per column (padded)
+constexpr int kRegsCtl = 32, kRegsWiden = 40, kRegsEpi = 184;  // launch: 96 per thread
 constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs;
 constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
-                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64;
-static_assert(kAccBufs * kNB <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
+                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64;
+static_assert((kWidenWGs & (kWidenWGs - 1)) == 0 && (kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
+static_assert((kOpStages & (kOpStages - 1)) == 0, "stage index wraps with a mask");
+static_assert(kAccBufs * kNT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
+static_assert(kI8StageBytes % 1024 == 0 && kPkStageBytes % 16 == 0, "alignment");
 static_assert(kSmemBytes <= 232448, "shared memory");
-static_assert(128 * kRegsCtl + 128 * kRegsWiden + 256 * kRegsEpi <= 65536, "registers");
+static_assert(128 * kRegsCtl + 128 * kWidenWGs * kRegsWiden + 256 * kRegsEpi <= kThreads * 96, "registers");
 
 struct Work {
-  int nt, mt;      // pair tile: 256 weight rows, 256 tokens
+  int nt, mt;      // pair tile: 256 weight rows, 192 tokens
   int kb0, kb1;
   int partial, units;
 };
@@ -73,6 +85,7 @@ __device__ __forceinline__ void work_begin(const GemmParams& p, WorkIter& it, in
   it.u = total * cp / npairs;
   it.u1 = total * (cp + 1) / npairs;
 }
+// Tiles are numbered token-tile fastest: pairs that run together share weight tiles in L2.
 __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Work& w, int cp, int npairs) {
   int tile;
   if (p.split == 0) {
@@ -99,7 +112,7 @@ __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Wor
 using namespace pair;
 
 template <bool BIAS, bool DUMP>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
     w4a4_gemm_pair_kernel(const GemmParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -110,6 +123,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
   constexpr uint32_t offScf = offPk + kPkStages * kPkStageBytes;
   constexpr uint32_t offBar = offScf + kScfSlots * kScfSlotBytes;
   constexpr uint32_t offTmemPtr = offBar + kNumBars * 8;
+  constexpr uint32_t offMagic = offTmemPtr + 64;       // 8 words of the magic bias (see epilogue)
   auto bar = [&](int i) { return smem_base + offBar + 8u * i; };
   constexpr int bPkFull = 0, bPkEmpty = bPkFull + kPkStages, bOpFull = bPkEmpty + kPkStages,
                 bOpEmpty = bOpFull + kOpStages, bScfFull = bOpEmpty + kOpStages,
@@ -130,152 +144,219 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
     // operand stage full: one elected arrive per widener warp of BOTH CTAs, on the leader's barrier
     for (int i = 0; i < kOpStages; ++i) { mbar_init(bar(bOpFull + i), 8); mbar_init(bar(bOpEmpty + i), 1); }
     for (int i = 0; i < kScfSlots; ++i) { mbar_init(bar(bScfFull + i), 128); mbar_init(bar(bScfEmpty + i), 8); }
-    // accumulator buffer empty: one elected arrive per epilogue warp of the owning warpgroup, both CTAs
-    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 8); }
+    // accumulator buffer empty: one elected arrive per epilogue warp of BOTH CTAs, on the leader's barrier
+    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 16); }
     fence_mbar_init();
   }
-  if (warp == 1) tmem_alloc_pair<512>(smem_base + offTmemPtr);
+  if (threadIdx.x < 8) reinterpret_cast<volatile uint32_t*>(smem_gen + offMagic)[threadIdx.x] = kMagicBits;
+  if (warp == kCtlWarp0 + 1) tmem_alloc_pair<512>(smem_base + offTmemPtr);
   tc_fence_before();
+  __syncthreads();
   cluster_sync_all();       // barriers of both CTAs initialised before any remote arrive / multicast
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + offTmemPtr);
+  if (tmem_base != 0) __trap();   // the whole TMEM (512 columns) is ours: lane 0, column 0
 
   WorkIter wit;
   Work w;
   work_begin(p, wit, cp, npairs);
+  auto stamp = [&](int ev, uint32_t k) {   // debug timeline: compiled in with -DAPEX4_TIMELINE only
+#ifdef APEX4_TIMELINE
+    if (p.tl != nullptr && blockIdx.x == 0 && k < 64) p.tl[ev * 64 + k] = clock64();
+#endif
+  };
 
-  // =========================================================================== producer
-  if (warp < 4) {
+  // =========================================================================== control warps
+  if (warp >= kCtlWarp0) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsCtl));
-    if (warp == 0 && lane == 0) {
+    // ------------------------------------------------------------------------- producer
+    // The whole warp runs the loop on warp-uniform values, one elected lane issues the copies;
+    // source pointers advance by a blob per k-block (no division, no 64-bit multiplies).
+    if (warp == kCtlWarp0) {
+      const bool el = elect_one();
       const int n_blobs = round_up(p.N, kTileRows) / kTileRows;
       const int m_blobs = round_up(p.M, kTileRows) / kTileRows;
       const uint32_t sc_bytes = gpk * 256;
-      uint32_t kbc = 0;
+      const size_t row_pitch = static_cast<size_t>(p.K / kBlockK) * kBlobBytes;   // bytes per blob row
+      const size_t srow_pitch = static_cast<size_t>(p.G) * kTileRows;               // FP16 scales per blob row
+      uint32_t kbc = 0, s = 0, pkpar = 0;
       while (work_next(p, wit, w, cp, npairs)) {
         const int wblob = 2 * w.nt + static_cast<int>(rank);
         const bool has_w = wblob < n_blobs;
-        const int a_blobs = min(2, m_blobs - 2 * w.mt);      // 128-token blobs of this tile
+        // this CTA's 96 token rows: up to two pieces of consecutive blobs
+        const int t0 = w.mt * kNT + static_cast<int>(rank) * kHalf;
+        const int ab0 = t0 >> 7, ar0 = t0 & 127;
+        const int n1 = ab0 < m_blobs ? min(kHalf, kTileRows - ar0) : 0;
+        const int n2 = (ab0 + 1 < m_blobs) ? kHalf - min(kHalf, kTileRows - ar0) : 0;
+        // token scales: the two blobs the 192-token tile touches
+        const int sb0 = (w.mt * kNT) >> 7;
+        const int s_blobs = min(2, m_blobs - sb0);
+        const int gfirst0 = g < kBlockK ? w.kb0 * gpk : w.kb0 / kbpg;
+        const uint8_t* wsrc = p.qW + wblob * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes;
+        const uint8_t* asrc = p.qA + ab0 * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes + ar0 * kRowBytes;
+        const __half* swsrc = p.sW + wblob * srow_pitch + static_cast<size_t>(gfirst0) * kTileRows;
+        const __half* sasrc = p.sA + sb0 * srow_pitch + static_cast<size_t>(gfirst0) * kTileRows;
+        const uint32_t bytes_data = (has_w ? kBlobBytes : 0) + (n1 + n2) * kRowBytes;
+        const uint32_t bytes_scales = sc_bytes * ((has_w ? 1 : 0) + s_blobs);
+        int kig = 0;
         for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-          const int s = kbc % kPkStages;
-          mbar_wait(bar(bPkEmpty + s), ((kbc / kPkStages) & 1) ^ 1);
+          mbar_wait(bar(bPkEmpty + s), ((pkpar >> s) & 1) ^ 1);
+          pkpar ^= 1u << s;
           const uint32_t st = smem_base + offPk + s * kPkStageBytes;
-          const bool has_scales = (kb % kbpg) == 0;
-          const int gfirst = g < kBlockK ? kb * gpk : kb / kbpg;
-          uint32_t bytes = (has_w ? kBlobBytes : 0) + a_blobs * 64 * kRowBytes;
-          if (has_scales) bytes += sc_bytes * ((has_w ? 1 : 0) + a_blobs);
-          mbar_arrive_expect_tx(bar(bPkFull + s), bytes);
-          if (has_w) bulk_g2s(st, p.qW + pt4_blob_offset(wblob, kb, p.K), kBlobBytes, bar(bPkFull + s));
-          for (int h = 0; h < a_blobs; ++h)   // half h of the tile = blob 2 mt + h; this CTA's 64 rows
-            bulk_g2s(st + kPkWBytes + h * 64 * kRowBytes,
-                     p.qA + pt4_blob_offset(2 * w.mt + h, kb, p.K) + rank * 64 * kRowBytes,
-                     64 * kRowBytes, bar(bPkFull + s));
-          if (has_scales) {
-            if (has_w)
-              bulk_g2s(st + kPkWBytes + kPkABytes,
-                       p.sW + (static_cast<size_t>(wblob) * p.G + gfirst) * kTileRows, sc_bytes,
-                       bar(bPkFull + s));
-            for (int h = 0; h < a_blobs; ++h)
-              bulk_g2s(st + kPkWBytes + kPkABytes + kPkSWBytes + h * sc_bytes,
-                       p.sA + (static_cast<size_t>(2 * w.mt + h) * p.G + gfirst) * kTileRows, sc_bytes,
-                       bar(bPkFull + s));
+          const uint32_t full = bar(bPkFull + s);
+          const bool has_scales = kig == 0;
+          if (el) {
+            stamp(0, kbc);
+            mbar_arrive_expect_tx(full, bytes_data + (has_scales ? bytes_scales : 0));
+            if (has_w) bulk_g2s(st, wsrc, kBlobBytes, full);
+            if (n1 > 0) bulk_g2s(st + kPkWBytes, asrc, n1 * kRowBytes, full);
+            if (n2 > 0)   // rows 0.. of the next blob
+              bulk_g2s(st + kPkWBytes + n1 * kRowBytes, asrc + row_pitch - ar0 * kRowBytes, n2 * kRowBytes, full);
+            if (has_scales) {
+              if (has_w) bulk_g2s(st + kPkWBytes + kPkABytes, swsrc, sc_bytes, full);
+              if (s_blobs > 0) bulk_g2s(st + kPkWBytes + kPkABytes + kPkSWBytes, sasrc, sc_bytes, full);
+              if (s_blobs > 1)
+                bulk_g2s(st + kPkWBytes + kPkABytes + kPkSWBytes + sc_bytes, sasrc + srow_pitch, sc_bytes, full);
+            }
           }
+          wsrc += kBlobBytes;
+          asrc += kBlobBytes;
+          if (has_scales) { swsrc += sc_bytes / 2; sasrc += sc_bytes / 2; }
+          kig = (kig == kbpg - 1) ? 0 : kig + 1;
+          s = (s == kPkStages - 1) ? 0 : s + 1;
         }
       }
     }
-    // ========================================================================= MMA issuer (leader)
-    else if (warp == 1 && lane == 0 && rank == 0) {
-      constexpr uint32_t idesc = umma_idesc_i8(256, kNB);
-      uint32_t kbc = 0, gc = 0;
-      const int ks_per_sub = 4 / gpk;
+    // ------------------------------------------------------------------------- debug observer
+#ifdef APEX4_TIMELINE
+    else if (warp == kCtlWarp0 + 2 && p.tl != nullptr && blockIdx.x == 0) {
+      uint32_t kbc = 0, s = 0, par = 0;
       while (work_next(p, wit, w, cp, npairs)) {
         for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-          const int t = kbc % kOpStages;
-          mbar_wait_cluster(bar(bOpFull + t), (kbc / kOpStages) & 1);
+          if (kbc < 64) { mbar_wait(bar(bPkFull + s), (par >> s) & 1); if (lane == 0) stamp(14, kbc); }
+          par ^= 1u << s;
+          s = (s == kPkStages - 1) ? 0 : s + 1;
+        }
+      }
+    }
+#endif
+    // ------------------------------------------------------------------------- MMA issuer (leader)
+    // Whole warp, warp-uniform values, one elected lane issues.  No division, no 64-bit descriptor
+    // arithmetic, stage / buffer parities kept as bit masks: the first version of this loop took
+    // ~2000 clk per k-block and was the bottleneck of the kernel (profiles/r1_gemm_v3_ncu.md).
+    else if (warp == kCtlWarp0 + 1 && rank == 0) {
+      const bool el = elect_one();
+      const uint32_t desc_lo0 = (((smem_base + offI8) & 0x3FFFFu) >> 4) | (1u << 16);
+      uint32_t kbc = 0, t = 0, oppar = 0, accpar = 0, buf0 = 0;
+      while (work_next(p, wit, w, cp, npairs)) {
+        int kig = 0;                                     // k-block inside the group
+        for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
+          mbar_wait(bar(bOpFull + t), (oppar >> t) & 1);
+          oppar ^= 1u << t;
           tc_fence_after();
-          const uint32_t a_tm = tmem_base + kTmemA0 + 32 * t;
-          const uint32_t b_sm = smem_base + offI8 + t * kI8StageBytes;
-          const bool first = (kb % kbpg) == 0;
-          const bool last = (kb % kbpg) == kbpg - 1;
-          for (int sub = 0; sub < gpk; ++sub) {
+          if (el) stamp(4, kbc);
+          const bool first = kig == 0;
+          const bool last = kig == kbpg - 1;
+          const uint32_t a_tm = kTmemA0 + 32 * t;        // the 512-column allocation starts at column 0
+          const uint32_t blo = desc_lo0 + t * (kI8StageBytes >> 4);
+          auto issue = [&](auto gpk_c) {
+            constexpr int GPK = decltype(gpk_c)::value;
+            constexpr int KS = 4 / GPK;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              const uint32_t u = (gc + sub) * 2 + h;
-              const uint32_t buf = u % kAccBufs;
+            for (int sub = 0; sub < GPK; ++sub) {
+              const uint32_t buf = (buf0 + sub) & 1;     // one accumulator buffer per group
               if (first) {
-                mbar_wait_cluster(bar(bAccEmpty + buf), (u / kAccBufs) & 1);
+                mbar_wait(bar(bAccEmpty + buf), (accpar >> buf) & 1);
+                accpar ^= 1u << buf;
                 tc_fence_after();
               }
-              const uint32_t d = tmem_base + buf * kNB;
-              const uint64_t bdesc = umma_desc_sw128(b_sm + h * (64 * kBlockK));
-              for (int ks = 0; ks < ks_per_sub; ++ks) {
-                const uint32_t kq = sub * ks_per_sub + ks;     // K=32 slice of the k-block
-                const uint32_t accum = BIAS ? 1u : ((first && ks == 0) ? 0u : 1u);
-                mma_i8_ts_pair(d, a_tm + 8 * kq, bdesc + 2 * kq, idesc, accum);
+#pragma unroll
+              for (int ks = 0; ks < KS; ++ks) {
+                const int kq = sub * KS + ks;            // K=32 slice of the k-block
+                if (el) {
+                  if (BIAS || ks != 0) mma_i8_ts_pair_lohi<true, kNT>(buf * kNT, a_tm + 8 * kq, blo + 2 * kq, 1u);
+                  else mma_i8_ts_pair_lohi<false, kNT>(buf * kNT, a_tm + 8 * kq, blo + 2 * kq, first ? 0u : 1u);
+                }
               }
-              if (last) tc_commit_pair(bar(bAccFull + buf), 3);
+              if (last && el) tc_commit_pair(bar(bAccFull + buf), 3);
             }
-          }
-          tc_commit_pair(bar(bOpEmpty + t), 3);
-          if (last) gc += gpk;
+          };
+          if (gpk == 1) issue(std::integral_constant<int, 1>{});
+          else if (gpk == 2) issue(std::integral_constant<int, 2>{});
+          else issue(std::integral_constant<int, 4>{});
+          if (el) tc_commit_pair(bar(bOpEmpty + t), 3);
+          if (el) stamp(5, kbc);
+          t = (t + 1) & (kOpStages - 1);
+          if (last) { buf0 = (buf0 + gpk) & 1; kig = 0; } else { ++kig; }
         }
       }
     }
   }
   // =========================================================================== wideners
-  else if (warp < 8) {
+  // Two warpgroups, k-blocks dealt alternately: one warp per SM sub-partition running a k-block's
+  // LDS -> LOP -> STS/STTM -> fence chain is latency-bound; two in flight overlap each other's drains.
+  else if (warp < kEpiWarp0) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsWiden));
-    const int r = threadIdx.x - 128;                    // weight row of this CTA's blob = TMEM lane
+    const int wwg = warp >> 2;                          // widener warpgroup
+    const int r = threadIdx.x & 127;                    // weight row of this CTA's blob = TMEM lane
     const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t wsw = (r >> 1) & 3;                  // chunk-slot swizzle of the packed row (PW4)
     const uint32_t flip = ((lane >> 2) & 1) * 16;       // see apex4_gemm.cu: bank spread of the two stores
     constexpr uint32_t kMask = 0xF0F0F0F0u;
-    uint32_t kbc = 0, gc = 0;
-    int pend_t = -1;                                    // operand stage written but not yet published
-    // Publishing stage t (fences + one elected arrive on the leader's barrier) is deferred until the
-    // loads of the next k-block are in flight, so the TMEM / shared-memory store drain overlaps them.
-    auto publish = [&](int t) {
-      fence_proxy_async_smem();
-      tmem_st_wait();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(bar(bOpFull + t), 0);
-    };
+    uint32_t kbc = 0, gc = 0, s = 0, t = 0, pkpar = 0, oppar = 0;
     while (work_next(p, wit, w, cp, npairs)) {
+      const int sa_off = (w.mt * kNT) & 127;            // tile token 0 inside its first scale blob
+      int kig = 0;
       for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-        const int s = kbc % kPkStages;
-        const int t = kbc % kOpStages;
-        mbar_wait(bar(bPkFull + s), (kbc / kPkStages) & 1);
-        const uint32_t pk_addr = smem_base + offPk + s * kPkStageBytes;
-        uint32_t wv[16];
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-          lds128(pk_addr + r * kRowBytes + ((j ^ wsw) << 4), wv[4 * j], wv[4 * j + 1], wv[4 * j + 2], wv[4 * j + 3]);
-        if (pend_t >= 0) publish(pend_t);
-        mbar_wait(bar(bOpEmpty + t), ((kbc / kOpStages) & 1) ^ 1);
+        const bool starts_group = kig == 0;
+        kig = (kig == kbpg - 1) ? 0 : kig + 1;
+        const uint32_t s_cur = s, t_cur = t;
+        s = (s == kPkStages - 1) ? 0 : s + 1;
+        t = (t + 1) & (kOpStages - 1);
+        const uint32_t pk_ph = (pkpar >> s_cur) & 1, op_ph = (oppar >> t_cur) & 1;
+        pkpar ^= 1u << s_cur;
+        oppar ^= 1u << t_cur;
+        if (static_cast<int>(kbc & (kWidenWGs - 1)) != wwg) {   // the other warpgroup's k-block
+          if (starts_group) gc += gpk;
+          continue;
+        }
+        mbar_wait(bar(bPkFull + s_cur), pk_ph);
+        if (r == 0) stamp(1, kbc);
+        const uint32_t pk_addr = smem_base + offPk + s_cur * kPkStageBytes;
+        uint32_t wv[8];
+        lds128(pk_addr + r * kRowBytes + ((0 ^ wsw) << 4), wv[0], wv[1], wv[2], wv[3]);
+        lds128(pk_addr + r * kRowBytes + ((1 ^ wsw) << 4), wv[4], wv[5], wv[6], wv[7]);
+        mbar_wait(bar(bOpEmpty + t_cur), op_ph ^ 1);
         tc_fence_after();
+        if (r == 0) stamp(2, kbc);
         // ---- weights: packed row r (64 bytes) -> 32 INT8 words -> TMEM columns of stage t
-        {
-          uint32_t o[32];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
+        for (int hh = 0; hh < 2; ++hh) {
+          uint32_t o[16];
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               o[8 * j + i] = rotl4(wv[4 * j + i]) & kMask;
               o[8 * j + 4 + i] = wv[4 * j + i] & kMask;
             }
           }
-          tmem_st_32x32(tmem_base + lane_addr + kTmemA0 + 32 * t, o);
+          if (hh == 0) {
+            lds128(pk_addr + r * kRowBytes + ((2 ^ wsw) << 4), wv[0], wv[1], wv[2], wv[3]);
+            lds128(pk_addr + r * kRowBytes + ((3 ^ wsw) << 4), wv[4], wv[5], wv[6], wv[7]);
+          }
+          tmem_st_32x16(tmem_base + lane_addr + kTmemA0 + 32 * t_cur + 16 * hh, o);
         }
-        // ---- tokens: packed byte offset o -> INT8 byte offsets 2o (lo nibbles), 2o+16 (hi)
+        if (r == 0) stamp(9, kbc);
+        // ---- tokens: 96 rows x 4 packed chunks; byte offset o -> INT8 offsets 2o (lo), 2o+16 (hi)
         {
-          uint32_t av[16];
+          uint32_t av[12];
 #pragma unroll
-          for (int x = 0; x < 4; ++x)
+          for (int x = 0; x < 3; ++x)
             lds128(pk_addr + kPkWBytes + (r + 128 * x) * 16, av[4 * x], av[4 * x + 1], av[4 * x + 2], av[4 * x + 3]);
-          const uint32_t dst0 = smem_base + offI8 + t * kI8StageBytes;
+          const uint32_t dst0 = smem_base + offI8 + t_cur * kI8StageBytes;
 #pragma unroll
-          for (int x = 0; x < 4; ++x) {
+          for (int x = 0; x < 3; ++x) {
             const uint32_t dst = dst0 + (r + 128 * x) * 32;
             const uint32_t l0 = rotl4(av[4 * x]) & kMask, h0 = av[4 * x] & kMask;
             const uint32_t l1 = rotl4(av[4 * x + 1]) & kMask, h1 = av[4 * x + 1] & kMask;
@@ -290,12 +371,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
             }
           }
         }
-        pend_t = t;
+        // ---- publish stage t: one elected arrive per warp on the leader's barrier
+        if (r == 0) stamp(10, kbc);
+        fence_proxy_async_smem();
+        if (r == 0) stamp(11, kbc);
+        tmem_st_wait();
+        if (r == 0) stamp(12, kbc);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(bar(bOpFull + t_cur), 0);
+        if (r == 0) stamp(3, kbc);
         // ---- scales of the groups that start in this k-block: FP16 -> FP32
-        if ((kb % kbpg) == 0) {
-          const uint8_t* pk = smem_gen + offPk + s * kPkStageBytes;
+        if (starts_group) {
+          const uint8_t* pk = smem_gen + offPk + s_cur * kPkStageBytes;
           const __half* sWh = reinterpret_cast<const __half*>(pk + kPkWBytes + kPkABytes);
-          const __half* sAh = sWh + kPkSWBytes / 2;
+          const __half* sAh = sWh + kPkSWBytes / 2;     // [blob 0/1][sub][128]
           for (int sub = 0; sub < gpk; ++sub, ++gc) {
             const int q = gc % kScfSlots;
             mbar_wait(bar(bScfEmpty + q), ((gc / kScfSlots) & 1) ^ 1);
@@ -308,35 +398,44 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 #pragma unroll
             for (int x = 0; x < 2; ++x) {
               const int col = r + 128 * x;                       // token of the tile
-              const int c = col & 15;
-              const int pos = (col & ~15) | (((c >> 1) & 3) << 2) | ((c >> 3) << 1) | (c & 1);
-              dstf[2 * kTileRows + pos] = __half2float(sAh[(x * gpk + sub) * kTileRows + r]);
+              if (col < kNT) {
+                const int mm = sa_off + col;                     // row in the tile's two scale blobs
+                const int c = col & 15;
+                const int pos = (col & ~15) | (((c >> 1) & 3) << 2) | ((c >> 3) << 1) | (c & 1);
+                dstf[2 * kTileRows + pos] = __half2float(sAh[((mm >> 7) * gpk + sub) * kTileRows + (mm & 127)]);
+              }
             }
             mbar_arrive(bar(bScfFull + q));
           }
         }
-        mbar_arrive(bar(bPkEmpty + s));
+        mbar_arrive(bar(bPkEmpty + s_cur));
+        if (r == 0) stamp(13, kbc);
       }
     }
-    if (pend_t >= 0) publish(pend_t);
   }
   // =========================================================================== epilogue
   else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsEpi));
-    const int h = (warp - 8) >> 2;                      // warpgroup = token half
+    const int h = (warp - kEpiWarp0) >> 2;              // warpgroup = token half
     const int lq = warp & 3;                            // TMEM lane quarter this warp may access
     const int q = lane >> 2, t = lane & 3;
-    const int epi_tid = threadIdx.x - 256;
+    const int epi_tid = threadIdx.x - 32 * kEpiWarp0;
     const uint32_t lane_addr = static_cast<uint32_t>(lq * 32) << 16;
     const int row0 = lq * 32 + q;                       // rows row0 + 8 i, i = 0..3
-
-    // completion #0 of every accEmpty barrier: buffer b is first used by unit u = b, half b & 1
+    // the magic bias in 8 registers, read through a volatile load so that ptxas keeps them resident
+    // instead of re-materialising 16 constants per tcgen05.st (IMAD.MOV on the FMA pipe)
+    uint32_t mg[8];
+    {
+      const uint32_t ma = smem_base + offMagic;
+      asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(mg[0]), "=r"(mg[1]), "=r"(mg[2]), "=r"(mg[3]) : "r"(ma));
+      asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(mg[4]), "=r"(mg[5]), "=r"(mg[6]), "=r"(mg[7]) : "r"(ma + 16));
+    }
+    // completion #0 of the accEmpty barriers: both buffers start out holding the magic bias
 #pragma unroll
     for (int b = 0; b < kAccBufs; ++b) {
-      if ((b & 1) != h) continue;
       if (BIAS) {
 #pragma unroll
-        for (int c = 0; c < kNB; c += 16) tmem_fill_32x16(tmem_base + lane_addr + b * kNB + c, kMagicBits);
+        for (int c = 0; c < kHalf; c += 8) tmem_st_32x8(tmem_base + lane_addr + b * kNT + h * kHalf + c, mg);
         tmem_st_wait();
       }
       tc_fence_before();
@@ -348,16 +447,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
     while (work_next(p, wit, w, cp, npairs)) {
       const int nkb = w.kb1 - w.kb0;
       const int ngroups = g < kBlockK ? nkb * gpk : nkb / kbpg;
-      uint64_t acc[64];                                 // [i][c][j] -> (i * 8 + c) * 2 + j
+      uint64_t acc[8 * kChunks];                        // [i][c][j] -> (i * kChunks + c) * 2 + j
 #pragma unroll
-      for (int i = 0; i < 64; ++i) acc[i] = 0ull;
+      for (int i = 0; i < 8 * kChunks; ++i) acc[i] = 0ull;
       const int n_glob0 = (2 * w.nt + static_cast<int>(rank)) * kTileRows + row0;
-      const int m_glob0 = w.mt * kNT + h * kNB + 2 * t;   // + 16 c + 8 j + e
+      const int m_glob0 = w.mt * kNT + h * kHalf + 2 * t;   // + 16 c + 8 j + e
 
       for (int gi = 0; gi < ngroups; ++gi, ++gc) {
         const int slot = gc % kScfSlots;
-        const uint32_t u = gc * 2 + h;
-        const uint32_t buf = u % kAccBufs;
+        const uint32_t buf = gc & 1;
         mbar_wait(bar(bScfFull + slot), (gc / kScfSlots) & 1);
         const uint32_t scf = smem_base + offScf + slot * kScfSlotBytes;
         uint64_t a2[4], b2[4];
@@ -368,22 +466,30 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
           a2[i] = pack_f2(af, af);
           b2[i] = pack_f2(bf, bf);
         }
-        const uint32_t sAf = scf + 2 * kTileRows * 4 + (h * kNB) * 4 + t * 16;   // + 64 c
-        mbar_wait(bar(bAccFull + buf), (u / kAccBufs) & 1);
+        const uint32_t sAf = scf + kTileRows * 8 + (h * kHalf) * 4 + t * 16;   // + 64 c
+        mbar_wait(bar(bAccFull + buf), (gc >> 1) & 1);
         tc_fence_after();
-        const uint32_t tb = tmem_base + lane_addr + buf * kNB;
+        if (epi_tid == 0) stamp(6, gc);
+        const uint32_t tb = tmem_base + lane_addr + buf * kNT + h * kHalf;
         uint32_t v[2][16];
+        uint64_t sq[2][2];                               // token scales of chunk c, c + 1
+        lds_2x64(sAf, sq[0][0], sq[0][1]);
         tmem_ld_16x256b_x2(tb, v[0]);
         tmem_ld_16x256b_x2(tb + (16u << 16), v[0] + 8);
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
+        for (int c = 0; c < kChunks; ++c) {
           uint32_t* vc = v[c & 1];
           tmem_ld_wait16(vc);
-          if constexpr (BIAS) tmem_fill_32x16(tb + 16 * c, kMagicBits);   // re-arm the chunk just read
-          if (c < 7) {
+          if (c < kChunks - 1) {                         // prefetch chunk c + 1, then re-arm chunk c
             tmem_ld_16x256b_x2(tb + 16 * (c + 1), v[(c + 1) & 1]);
             tmem_ld_16x256b_x2(tb + (16u << 16) + 16 * (c + 1), v[(c + 1) & 1] + 8);
-          } else {                                       // buffer fully read (and re-armed): hand it back
+            lds_2x64(sAf + 64 * (c + 1), sq[(c + 1) & 1][0], sq[(c + 1) & 1][1]);
+          }
+          if constexpr (BIAS) {
+            tmem_st_32x8(tb + 16 * c, mg);
+            tmem_st_32x8(tb + 16 * c + 8, mg);
+          }
+          if (c == kChunks - 1) {                        // buffer fully read (and re-armed): hand it back
             if constexpr (BIAS) tmem_st_wait();
             tc_fence_before();
             __syncwarp();
@@ -406,25 +512,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
                   }
                 }
           }
-          uint64_t s01, s23;
-          lds_2x64(sAf + 64 * c, s01, s23);              // token scales of columns {2t,2t+1}, {8+2t,9+2t}
+          const uint64_t s01 = sq[c & 1][0], s23 = sq[c & 1][1];   // columns {2t,2t+1}, {8+2t,9+2t}
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int rb = 8 * (i >> 1) + 2 * (i & 1);
             uint64_t t0, t1;
             if constexpr (BIAS) {
-              t0 = fma2(pack_u2(vc[rb], vc[rb + 1]), a2[i], b2[i]);
-              t1 = fma2(pack_u2(vc[rb + 4], vc[rb + 5]), a2[i], b2[i]);
+              t0 = fma2v(pack_u2(vc[rb], vc[rb + 1]), a2[i], b2[i]);
+              t1 = fma2v(pack_u2(vc[rb + 4], vc[rb + 5]), a2[i], b2[i]);
             } else {
               t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[rb])), __int2float_rn(static_cast<int>(vc[rb + 1]))), a2[i]);
               t1 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[rb + 4])), __int2float_rn(static_cast<int>(vc[rb + 5]))), a2[i]);
             }
-            acc[(i * 8 + c) * 2] = fma2(t0, s01, acc[(i * 8 + c) * 2]);
-            acc[(i * 8 + c) * 2 + 1] = fma2(t1, s23, acc[(i * 8 + c) * 2 + 1]);
+            acc[(i * kChunks + c) * 2] = fma2(t0, s01, acc[(i * kChunks + c) * 2]);
+            acc[(i * kChunks + c) * 2 + 1] = fma2(t1, s23, acc[(i * kChunks + c) * 2 + 1]);
           }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(bScfEmpty + slot));
+        if (epi_tid == 0) stamp(7, gc);
       }
 
       // ---- a7 (cast + store) or a6 (cross-pair reduce through the FP32 workspace)
@@ -435,11 +541,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
             const int n = n_glob0 + 8 * i;
             if (n >= p.N) continue;
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
+            for (int c = 0; c < kChunks; ++c)
 #pragma unroll
               for (int j = 0; j < 2; ++j) {
                 float f0, f1;
-                unpack_f2(acc[(i * 8 + c) * 2 + j], f0, f1);
+                unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
                 const int m = m_glob0 + 16 * c + 8 * j;
                 if (p.out_f32) {
                   float* y = static_cast<float*>(p.Y);
@@ -453,16 +559,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
               }
           }
         } else {
+          // a6: FP32 partial sums meet in the workspace (red.add at L2); the CTA that completes its
+          // half of the tile casts, stores and leaves the workspace zero-filled again (PAPER.md:230
+          // "inter-SM global reduction").
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int n = n_glob0 + 8 * i;
             if (n >= p.N) continue;
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
+            for (int c = 0; c < kChunks; ++c)
 #pragma unroll
               for (int j = 0; j < 2; ++j) {
                 float f0, f1;
-                unpack_f2(acc[(i * 8 + c) * 2 + j], f0, f1);
+                unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
                 const int m = m_glob0 + 16 * c + 8 * j;
                 if (m < p.M) atomicAdd(p.ws + static_cast<size_t>(m) * p.N + n, f0);
                 if (m + 1 < p.M) atomicAdd(p.ws + static_cast<size_t>(m + 1) * p.N + n, f1);
@@ -488,7 +597,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
               const int n = n_glob0 + 8 * i;
               if (n >= p.N) continue;
 #pragma unroll 4
-              for (int cj = 0; cj < 16; ++cj)
+              for (int cj = 0; cj < 2 * kChunks; ++cj)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                   const int m = m_glob0 + 8 * cj + e;
@@ -511,7 +620,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
   // ---- teardown: nobody leaves while the peer may still signal this CTA's barriers or read its
   // shared memory / TMEM through the pair MMA
   cluster_sync_all();
-  if (warp == 1) {
+  if (warp == kCtlWarp0 + 1) {
     tc_fence_after();
     tmem_dealloc_pair<512>(tmem_base);
   }

@@ -154,6 +154,19 @@ __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&v
       "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
       : "memory");
 }
+__device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+      "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+      "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_32x8(uint32_t taddr, const uint32_t (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+               "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+               : "memory");
+}
 // the same 32-bit value into 16 / 8 consecutive columns of the warp's 32 lanes
 __device__ __forceinline__ void tmem_fill_32x16(uint32_t taddr, uint32_t c) {
   asm volatile(
@@ -170,6 +183,12 @@ __device__ __forceinline__ void tmem_st_wait() {
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
+// kind::i8 instruction descriptor: S32 accumulate (c_format 2 at [4,6)), signed 8-bit A/B (1 at
+// [7,10) and [10,13)), both K-major, no saturate, N>>3 at [17,23), M>>4 at [24,29).
+__host__ __device__ constexpr uint32_t umma_idesc_i8(uint32_t M, uint32_t N) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+}
+
 // ------------------------------------------------------------------ CTA pair (cluster of 2, cta_group::2)
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
@@ -180,12 +199,15 @@ __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
   asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// arrive (count 1) on the mbarrier at the same shared-memory offset in CTA `rank` of the cluster
+// arrive (count 1) on the mbarrier at the same shared-memory offset in CTA `rank` of the cluster.
+// Plain (release.cta) arrive, as in CUTLASS' ClusterBarrier: `.release.cluster` compiles to
+// MEMBAR.ALL.GPU + ERRBAR (thousands of cycles on the hand-off path, profiles/r1_gemm_v3_ncu.md); what
+// the peer must see is ordered by the tcgen05 fences and fence.proxy.async issued before the arrive.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank) {
   asm volatile(
       "{\n\t.reg .b32 ra;\n\t"
       "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
-      "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar),
+      "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar),
       "r"(rank)
       : "memory");
 }
@@ -234,6 +256,41 @@ __device__ __forceinline__ void mma_i8_ts_pair(uint32_t d_tmem, uint32_t a_tmem,
       "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// Same, for a warp-uniform issue loop: descriptor passed as two 32-bit halves (hi is a constant of the
+// SWIZZLE_128B K-major layout), instruction descriptor a compile-time constant; ACC = accumulate
+// unconditionally, else `accumulate` decides.
+template <bool ACC, int N>
+__device__ __forceinline__ void mma_i8_ts_pair_lohi(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo,
+                                                    uint32_t accumulate) {
+  constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
+  constexpr uint32_t idesc = umma_idesc_i8(256, N);
+  if constexpr (ACC) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 bd;\n\t"
+        "mov.b64 bd, {%2, %3};\n\t"
+        "setp.eq.b32 p, 0, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], [%1], bd, %4, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "r"(b_lo), "n"(kDescHi), "n"(idesc)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 bd;\n\t"
+        "mov.b64 bd, {%2, %3};\n\t"
+        "setp.ne.b32 p, %5, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], [%1], bd, %4, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "r"(b_lo), "n"(kDescHi), "n"(idesc), "r"(accumulate)
+        : "memory");
+  }
+}
+__device__ __forceinline__ bool elect_one() {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok));
+  return ok != 0;
+}
 // arrive on the mbarrier at this offset in every CTA of `mask` once all prior tcgen05 ops are done
 __device__ __forceinline__ void tc_commit_pair(uint32_t bar, uint16_t mask) {
   asm volatile(
@@ -276,11 +333,6 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
   d |= static_cast<uint64_t>(2) << 61;            // SWIZZLE_128B
   return d;
 }
-// kind::i8 instruction descriptor: S32 accumulate (c_format 2 at [4,6)), signed 8-bit A/B (1 at
-// [7,10) and [10,13)), both K-major, no saturate, N>>3 at [17,23), M>>4 at [24,29).
-__host__ __device__ constexpr uint32_t umma_idesc_i8(uint32_t M, uint32_t N) {
-  return (2u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
-}
 
 // ------------------------------------------------------------------ 128-bit shared-memory access
 __device__ __forceinline__ void lds128(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
@@ -316,6 +368,13 @@ __device__ __forceinline__ void unpack_f2(uint64_t v, float& lo, float& hi) {
 __device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
   uint64_t d;
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+// volatile twin: keeps its place among the other volatile asms (tcgen05.ld / wait), so that a
+// prefetching tcgen05.ld written before the arithmetic of the previous chunk is issued before it
+__device__ __forceinline__ uint64_t fma2v(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
   return d;
 }
 __device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
