@@ -460,12 +460,22 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemm_kernel(const GemmParams
             if (done) {
               __threadfence();
               if (n_glob < p.N) {
-#pragma unroll 4
+#pragma unroll
+                for (int j = 0; j < CPT; j += 2) {       // all loads first, then the stores
+                  const int m = m_glob0 + j;
+                  float f0 = 0.f, f1 = 0.f;
+                  if (m < p.M) f0 = __ldcg(p.ws + static_cast<size_t>(m) * p.N + n_glob);
+                  if (m + 1 < p.M) f1 = __ldcg(p.ws + static_cast<size_t>(m + 1) * p.N + n_glob);
+                  acc[j / 2] = pack_f2(f0, f1);
+                }
+#pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                   const int m = m_glob0 + j;
                   if (m < p.M) {
                     const size_t idx = static_cast<size_t>(m) * p.N + n_glob;
-                    const float vsum = __ldcg(p.ws + idx);
+                    float f0, f1;
+                    unpack_f2(acc[j / 2], f0, f1);
+                    const float vsum = (j & 1) ? f1 : f0;
                     __stcg(p.ws + idx, 0.f);
                     if (p.out_f32) static_cast<float*>(p.Y)[idx] = vsum;
                     else static_cast<__half*>(p.Y)[idx] = __float2half_rn(vsum);

@@ -443,8 +443,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + b), 0);
     }
 
-    uint32_t gc = 0;
+    uint32_t gc = 0, item = 0;
     while (work_next(p, wit, w, cp, npairs)) {
+      if (epi_tid == 0) stamp(15, item * 4);
       const int nkb = w.kb1 - w.kb0;
       const int ngroups = g < kBlockK ? nkb * gpk : nkb / kbpg;
       uint64_t acc[8 * kChunks];                        // [i][c][j] -> (i * kChunks + c) * 2 + j
@@ -534,6 +535,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       }
 
       // ---- a7 (cast + store) or a6 (cross-pair reduce through the FP32 workspace)
+      if (epi_tid == 0) stamp(15, item * 4 + 1);
       if (p.Y != nullptr) {
         if (!w.partial) {
 #pragma unroll
@@ -578,6 +580,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
               }
           }
           __threadfence();
+          if (epi_tid == 0) stamp(15, item * 4 + 2);
           int* flag = reinterpret_cast<int*>(smem_gen + offTmemPtr + 8);
           asm volatile("bar.sync 1, 256;" ::: "memory");
           if (epi_tid == 0) {
@@ -591,28 +594,46 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
           const int done = *flag;
           asm volatile("bar.sync 1, 256;" ::: "memory");   // flag may be rewritten by the next item
           if (done) {
+            // all loads first (the running sums are dead: their registers hold the tile), then the
+            // stores -- a load/store/load chain here costs one L2 round trip per element
             __threadfence();
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const int n = n_glob0 + 8 * i;
+#pragma unroll
+              for (int cj = 0; cj < 2 * kChunks; ++cj) {
+                const int m = m_glob0 + 8 * cj;
+                float f0 = 0.f, f1 = 0.f;
+                if (n < p.N && m < p.M) f0 = __ldcg(p.ws + static_cast<size_t>(m) * p.N + n);
+                if (n < p.N && m + 1 < p.M) f1 = __ldcg(p.ws + static_cast<size_t>(m + 1) * p.N + n);
+                acc[i * 2 * kChunks + cj] = pack_f2(f0, f1);
+              }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int n = n_glob0 + 8 * i;
               if (n >= p.N) continue;
-#pragma unroll 4
-              for (int cj = 0; cj < 2 * kChunks; ++cj)
+#pragma unroll
+              for (int cj = 0; cj < 2 * kChunks; ++cj) {
+                float f[2];
+                unpack_f2(acc[i * 2 * kChunks + cj], f[0], f[1]);
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                   const int m = m_glob0 + 8 * cj + e;
                   if (m < p.M) {
                     const size_t idx = static_cast<size_t>(m) * p.N + n;
-                    const float vsum = __ldcg(p.ws + idx);
                     __stcg(p.ws + idx, 0.f);
-                    if (p.out_f32) static_cast<float*>(p.Y)[idx] = vsum;
-                    else static_cast<__half*>(p.Y)[idx] = __float2half_rn(vsum);
+                    if (p.out_f32) static_cast<float*>(p.Y)[idx] = f[e];
+                    else static_cast<__half*>(p.Y)[idx] = __float2half_rn(f[e]);
                   }
                 }
+              }
             }
           }
         }
       }
+      if (epi_tid == 0) stamp(15, item * 4 + 3);
+      ++item;
     }
     tc_fence_before();
   }
