@@ -68,10 +68,11 @@ struct Dispatch {
   int split;   // stream-K work distribution (needs the workspace)
   int grid;
   int upt, kbu, tiles_m, tiles_n;
+  int rows8, mt;   // nt == 0: decode (stream) kernel, 8-row groups per warp and m16 token tiles
 };
 
 // test hook (apex4_debug_set_dispatch): -1 = automatic
-int g_force_nt = -1, g_force_split = -1, g_force_grid = -1;
+int g_force_nt = -1, g_force_split = -1, g_force_grid = -1;   // g_force_nt == 0 forces the decode kernel
 long long* g_timeline = nullptr;
 
 Dispatch choose_dispatch(int M, int N, int K, int g) {
@@ -80,12 +81,31 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
   d.kbu = g > kBlockK ? g / kBlockK : 1;   // indivisible k unit: a whole group, at least a k-block
   d.upt = KB / d.kbu;
   d.bias = g <= kBlockK;
+  d.rows8 = d.mt = 0;
+  const bool gemv_ok = M <= 64 && g == kBlockK;   // larger groups: the tile kernel keeps one rounding per group (R12)
   if (g_force_nt > 0) d.nt = g_force_nt;
+  else if (gemv_ok) d.nt = 0;
   else if (M <= 16) d.nt = 16;
   else if (M <= 32) d.nt = 32;
   else if (M <= 64) d.nt = 64;
   else if (M <= 128) d.nt = 128;
   else d.nt = 256;
+  if (d.nt == 0) {
+    // decode kernel: a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
+    d.bias = 0;
+    d.mt = (M + 15) / 16;
+    d.rows8 = 1;
+    d.tiles_m = 1;
+    d.tiles_n = (N + 7) / 8;
+    d.grid = g_force_grid > 0 ? g_force_grid : gemm_max_ctas();
+    if (d.grid > d.tiles_n) d.grid = d.tiles_n;
+    const int per_cta = (d.tiles_n + d.grid - 1) / d.grid;
+    const int max_batch = gemv_max_batch(d.mt);
+    d.upt = per_cta < max_batch ? per_cta : max_batch;     // row blocks per shared-memory batch
+    if (g_force_nt == 0 && g_force_split > 0 && g_force_split < d.upt) d.upt = g_force_split;   // test hook
+    d.split = 0;
+    return d;
+  }
   const bool pair = d.nt == 256;
   d.tiles_m = pair ? (M + kPairTokens - 1) / kPairTokens : (M + d.nt - 1) / d.nt;
   d.tiles_n = pair ? (N + 2 * kTileRows - 1) / (2 * kTileRows) : (N + kTileRows - 1) / kTileRows;
@@ -109,6 +129,7 @@ size_t counters_bytes(const Dispatch& d) {
 
 cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
   const cudaError_t e = d.nt == 256 ? launch_gemm_pair(p, d.bias, dump, d.grid, st)
+                        : d.nt == 0 ? launch_gemv(p, d.mt, dump, d.grid, st)
                                     : launch_gemm(p, d.nt, d.bias, dump, d.grid, st);
   if (e != cudaSuccess && getenv("APEX4_VERBOSE"))
     fprintf(stderr, "apex4: GEMM launch (tile %d, grid %d) failed: %s\n", d.nt, d.grid, cudaGetErrorString(e));

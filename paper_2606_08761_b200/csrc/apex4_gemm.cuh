@@ -41,4 +41,9 @@ constexpr int kPairTokens = 192;   // tokens per CTA-pair tile
 cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st);
 int gemm_max_pairs();
 
+// Decode regime (apex4_gemv.cu): M <= 64, g a multiple of 128, no workspace.  tiles_n = 8-row row blocks,
+// upt = row blocks per shared-memory batch (<= gemv_max_batch(mt)), kbu = k-blocks per group.
+cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st);
+int gemv_max_batch(int mt);
+
 }  // namespace apex4
