@@ -94,13 +94,13 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
     // decode kernel: a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
     d.bias = 0;
     d.mt = (M + 15) / 16;
-    d.rows8 = 1;
+    d.rows8 = d.mt >= 3 ? 1 : 0;     // 1: register-ring kernel (3-4 token tiles), 0: bulk-copy staged kernel
     d.tiles_m = 1;
     d.tiles_n = (N + 7) / 8;
     d.grid = g_force_grid > 0 ? g_force_grid : gemm_max_ctas();
     if (d.grid > d.tiles_n) d.grid = d.tiles_n;
     const int per_cta = (d.tiles_n + d.grid - 1) / d.grid;
-    const int max_batch = gemv_max_batch(d.mt);
+    const int max_batch = d.rows8 ? gemv_ring_max_batch(d.mt) : gemv_max_batch(d.mt);
     d.upt = per_cta < max_batch ? per_cta : max_batch;     // row blocks per shared-memory batch
     if (g_force_nt == 0 && g_force_split > 0 && g_force_split < d.upt) d.upt = g_force_split;   // test hook
     d.split = 0;
@@ -129,7 +129,7 @@ size_t counters_bytes(const Dispatch& d) {
 
 cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
   const cudaError_t e = d.nt == 256 ? launch_gemm_pair(p, d.bias, dump, d.grid, st)
-                        : d.nt == 0 ? launch_gemv(p, d.mt, dump, d.grid, st)
+                        : d.nt == 0 ? (d.rows8 ? launch_gemv_ring(p, d.mt, dump, d.grid, st) : launch_gemv(p, d.mt, dump, d.grid, st))
                                     : launch_gemm(p, d.nt, d.bias, dump, d.grid, st);
   if (e != cudaSuccess && getenv("APEX4_VERBOSE"))
     fprintf(stderr, "apex4: GEMM launch (tile %d, grid %d) failed: %s\n", d.nt, d.grid, cudaGetErrorString(e));

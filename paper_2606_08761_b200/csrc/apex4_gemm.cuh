@@ -45,5 +45,8 @@ int gemm_max_pairs();
 // upt = row blocks per shared-memory batch (<= gemv_max_batch(mt)), kbu = k-blocks per group.
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st);
 int gemv_max_batch(int mt);
+// 32 < M <= 64 (apex4_gemv_ring.cu): same parameters, register-ring staging
+cudaError_t launch_gemv_ring(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st);
+int gemv_ring_max_batch(int mt);
 
 }  // namespace apex4

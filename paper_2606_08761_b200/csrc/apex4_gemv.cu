@@ -1,21 +1,25 @@
-// apex4_gemv.cu -- a2..a7 of the hot path for the decode regime (M <= 64, g a multiple of 128): the
+// apex4_gemv.cu -- a2..a7 of the hot path for the decode regime (M <= 32, g = 128): the
 // weights are read once from HBM and every byte is used M times, so the kernel is a weight STREAM:
 // no shared-memory staging of operands, no TMEM, no cross-CTA exchange, no workspace.
 //
-//   * A CTA (16 warps) owns a contiguous range of 8-row weight groups ("row blocks") and ALL of K.
-//     Warp w owns the k-blocks [KB w / 16, KB (w+1) / 16): its token fragments (the m16 operand of
-//     mma.sync.m16n8k32.s8) depend on k only, so they are loaded from the PT4 layout and widened ONCE
-//     per pass (C k-blocks at a time) and stay in registers while the warp walks down the row blocks.
-//   * Per row block and k-block a warp issues ONE fully coalesced 512-byte weight load (lane (q, t) =
-//     row q, the 16-byte packed chunk that holds K slice t) straight into a register ring of depth D
-//     (D - 1 loads in flight per warp, ~4 KB; 64 KB per SM), widens the four packed words with two logic
-//     ops each (16 x code, apex4_layout.cuh) and feeds them to four MMAs.  MMA i takes word i of every
-//     lane: its 32 k are {32 t + 4 i + e, 32 t + 16 + 4 i + e}; any k order inside a group gives the
-//     same exact INT32 sum and the token fragments use the very same lane -> k assignment.
-//   * Each k-block's INT32 sum is converted, multiplied by sW/256 (operands are 16 q) and by sA of its
-//     group and added to the warp's FP32 partial (Eq. 8 is linear in the per-k-block sums, so a group
-//     larger than a k-block needs no special case); partials go to a warp-private shared-memory slot
-//     and are reduced across the 16 warps once per batch of row blocks, then cast and stored (a6, a7).
+//   * A CTA (16 warps) owns a contiguous range of 8-row weight groups ("row blocks"), processed in
+//     batches of RBB row blocks, and ALL of K.  Warp w owns the k-blocks [KB w / 16, KB (w+1) / 16).
+//   * Operand staging is warp-private: for each of its k-blocks the warp's elected lane issues 1-D bulk
+//     async copies (cp.async.bulk, TMA engine) of the batch's weight rows (RBB x 512 contiguous bytes of
+//     the PW4 blob), the token rows, and both scale vectors into one of the warp's two shared-memory
+//     stages, completion counted on an mbarrier.  16 warps x 2 stages x ~4.7 KB = 150 KB per SM are in
+//     flight with no register cost (a register ring held only 57 KB and cost one HBM round trip per 7
+//     units and warp: 15 us; profiles/r1_gemv_ncu.md).  No cross-warp hand-off: the warp that issued a
+//     stage is the one that consumes it and re-arms it.
+//   * Consumption: lane (q, t) reads the 16-byte packed chunk that holds K slice t of row q (one
+//     conflict-free LDS.128 per row block), widens the four words with two logic ops each (16 x code,
+//     apex4_layout.cuh) and feeds them to four mma.sync.m16n8k32.s8 (tokens = m16, 8 weight rows = n8).
+//     MMA i takes word i of every lane: its 32 k are {32 t + 4 i + e, 32 t + 16 + 4 i + e}; any k order
+//     inside a group gives the same exact INT32 sum and the token fragments (widened once per k-block,
+//     reused by every row block) use the very same lane -> k assignment.
+//   * Each k-block's INT32 sum is converted, multiplied by sW/256 (operands are 16 q) and sA and added
+//     to the warp's FP32 partial sums (registers, one set per row block of the batch); once per batch
+//     the partials of the 16 warps are reduced through shared memory, cast and stored (a6, a7).
 // Tensor cores here are the legacy warp-level path on purpose: at M <= 64 the MMA work is < 2 % of the
 // HBM time and a tcgen05 pipeline (bulk copy -> widen -> TMEM -> MMA -> TMEM load) only adds latency
 // (profiles/r1_gemm_v2_ncu.md: 48 us at M = 16 against 5.3 us of HBM time).
@@ -32,7 +36,7 @@ namespace gemv {
 constexpr int kWarps = 16;
 constexpr int kThreads = 32 * kWarps;
 constexpr uint32_t kMask = 0xF0F0F0F0u;
-constexpr int kSlotBudget = 192 * 1024;                 // shared memory for the partial sums of a batch
+constexpr int kStages = 2;                              // warp-private operand stages
 
 __device__ __forceinline__ uint4 ldg_stream(const uint8_t* p) {   // weights: read once, keep out of L1
   uint4 v;
@@ -67,89 +71,126 @@ __device__ __forceinline__ uint32_t word(const uint4& v, int i) {
 
 using namespace gemv;
 
-// MT: m16 token tiles (M <= 16 MT); C: k-blocks whose token fragments a warp keeps in registers.
-// p.tiles_n = 8-row row blocks, p.upt = row blocks per batch (shared-memory slots), p.kbu = k-blocks
-// per group.
-template <int MT, int C, bool DUMP>
+
+// MT: m16 token tiles (M <= 16 MT).  p.tiles_n = 8-row row blocks; p.kbu = k-blocks per group.
+template <int MT>
+struct GemvCfg {
+  static constexpr int RBB = MT == 1 ? 7 : MT == 2 ? 4 : MT == 3 ? 2 : 1;         // row blocks per batch
+  static constexpr int kWBytes = RBB * 8 * kRowBytes;                // weight rows of a k-block
+  static constexpr int kABytes = MT * 16 * kRowBytes;                // token rows of a k-block
+  static constexpr int kSWBytes = (RBB * 16 + 15) / 16 * 16;         // FP16 weight scales of the batch rows
+  static constexpr int kSABytes = MT * 32;                           // FP16 token scales
+  static constexpr int kStageBytes = kWBytes + kABytes + kSWBytes + kSABytes;
+  static constexpr int kPartBytes = RBB * kWarps * MT * 512;         // FP32 partial sums of a batch
+  static constexpr int kSmemBytes = 128 + kPartBytes + kWarps * kStages * kStageBytes + kWarps * kStages * 8;
+  static_assert(kStageBytes % 16 == 0 && kSmemBytes <= 232448, "shared memory");
+};
+
+template <int MT, bool DUMP>
 __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams p) {
-  constexpr int D = MT == 1 ? 8 : 6;                    // register ring depth (D - 1 loads in flight)
-  extern __shared__ float4 slots[];                     // [row block of the batch][warp][MT][lane]
+  using Cfg = GemvCfg<MT>;
+  constexpr int RBB = Cfg::RBB;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
+  uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+  float4* part = reinterpret_cast<float4*>(smem_gen);                // [row block][warp][MT][lane]
+  constexpr uint32_t offStage = Cfg::kPartBytes;
+  constexpr uint32_t offBar = offStage + kWarps * kStages * Cfg::kStageBytes;
+
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int q = lane >> 2, t = lane & 3;
   const int KB = p.K / kBlockK;
   const int kbw0 = KB * w / kWarps, kbw1 = KB * (w + 1) / kWarps;    // this warp's k-blocks
+  const int nkw = kbw1 - kbw0;
   const int rb0 = static_cast<int>(static_cast<long long>(p.tiles_n) * blockIdx.x / gridDim.x);
   const int rb1 = static_cast<int>(static_cast<long long>(p.tiles_n) * (blockIdx.x + 1) / gridDim.x);
-  const int rbB = p.upt;
   const size_t row_pitch = static_cast<size_t>(KB) * kBlobBytes;
   const bool swap = (q & 1) != 0;                       // odd token rows: lo / hi nibbles exchanged (PT4)
-  // byte offset of this lane's 16-byte chunk (K slice t of row q) inside an 8-row group of a blob
+  // byte offset of this lane's 16-byte chunk (K slice t of row q) inside an 8-row group
   const uint32_t lane_off = q * kRowBytes + ((t ^ ((q >> 1) & 3)) << 4);
+  const uint32_t my_stage0 = smem_base + offStage + w * kStages * Cfg::kStageBytes;
+  const uint32_t my_bar0 = smem_base + offBar + w * kStages * 8;
+  if (lane == 0) {
+    for (int s = 0; s < kStages; ++s) mbar_init(my_bar0 + 8 * s, 1);
+    fence_mbar_init();
+  }
+  __syncwarp();
 
-  for (int b0 = rb0; b0 < rb1; b0 += rbB) {
-    const int nb = min(rbB, rb1 - b0);
-    for (int i = 0; i < nb; ++i)
-#pragma unroll
-      for (int mi = 0; mi < MT; ++mi) slots[((i * kWarps + w) * MT + mi) * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+  // ---- issue cursor: (batch start row block, k-block index of this warp), flattened, k fastest
+  int ib0 = rb0, ij = 0, islot = 0;
+  auto issue_next = [&]() {                             // elected lane: copies of one stage
+    if (ib0 >= rb1 || nkw == 0) return;
+    const int nb = min(RBB, rb1 - ib0);
+    const int kb = kbw0 + ij;
+    const uint32_t st = my_stage0 + islot * Cfg::kStageBytes;
+    const uint32_t full = my_bar0 + 8 * islot;
+    const int row_a = ib0 * 8, row_b = row_a + nb * 8;                 // weight rows of the batch
+    const int tile_a = row_a >> 7;
+    const int split_row = min(row_b, (tile_a + 1) << 7);               // rows [row_a, split_row) in tile_a
+    const int n1 = split_row - row_a, n2 = row_b - split_row;
+    const int gm = kb / p.kbu;
+    mbar_arrive_expect_tx(full, (n1 + n2) * kRowBytes + Cfg::kABytes + (n1 + n2) * 2 + Cfg::kSABytes);
+    bulk_g2s(st, p.qW + tile_a * row_pitch + static_cast<size_t>(kb) * kBlobBytes + (row_a & 127) * kRowBytes,
+             n1 * kRowBytes, full);
+    bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes,
+             p.sW + (static_cast<size_t>(tile_a) * p.G + gm) * kTileRows + (row_a & 127), n1 * 2, full);
+    if (n2 > 0) {
+      bulk_g2s(st + n1 * kRowBytes, p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kb) * kBlobBytes,
+               n2 * kRowBytes, full);
+      bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + n1 * 2,
+               p.sW + (static_cast<size_t>(tile_a + 1) * p.G + gm) * kTileRows, n2 * 2, full);
+    }
+    bulk_g2s(st + Cfg::kWBytes, p.qA + static_cast<size_t>(kb) * kBlobBytes, Cfg::kABytes, full);
+    bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, p.sA + static_cast<size_t>(gm) * kTileRows,
+             Cfg::kSABytes, full);
+    islot = islot + 1 == kStages ? 0 : islot + 1;
+    if (++ij == nkw) { ij = 0; ib0 += RBB; }
+  };
+  if (lane == 0)
+    for (int s = 0; s < kStages; ++s) issue_next();
 
-    float yfr[MT][4];
-    // One pass = CC k-blocks (kc .. kc + CC - 1) against every row block of the batch.  CC is a
-    // compile-time constant so that every register index below is static (a run-time choice of the
-    // token fragment compiled to predicated copies of every MMA: 140 instructions per 512-byte unit).
-    auto pass = [&](int kc, auto cc_c) {
-      constexpr int CC = decltype(cc_c)::value;
-      // ---- token fragments and token scales (registers, reused by every row block)
-      uint32_t af[CC][MT][4][4];
-      float sa[CC][MT][2];
-      int gam[CC];
+  uint32_t par = 0;                                     // phase parity of the warp's stage barriers
+  int cslot = 0;
+  for (int b0 = rb0; b0 < rb1; b0 += RBB) {
+    const int nb = min(RBB, rb1 - b0);
+    float yf[RBB][MT][4];
 #pragma unroll
-      for (int c = 0; c < CC; ++c) {
-        const int kb = kc + c;
-        gam[c] = kb / p.kbu;
-        const uint8_t* ap = p.qA + static_cast<size_t>(kb) * kBlobBytes + lane_off;
+    for (int i = 0; i < RBB; ++i)
 #pragma unroll
-        for (int mi = 0; mi < MT; ++mi) {
-          const uint4 x0 = ldg_cached(ap + (16 * mi) * kRowBytes);
-          const uint4 x1 = ldg_cached(ap + (16 * mi + 8) * kRowBytes);
+      for (int mi = 0; mi < MT; ++mi)
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const uint32_t l0 = rotl4(word(x0, i)) & kMask, h0 = word(x0, i) & kMask;
-            const uint32_t l1 = rotl4(word(x1, i)) & kMask, h1 = word(x1, i) & kMask;
-            af[c][mi][i][0] = swap ? h0 : l0; af[c][mi][i][2] = swap ? l0 : h0;   // token q: k lo / hi half
-            af[c][mi][i][1] = swap ? h1 : l1; af[c][mi][i][3] = swap ? l1 : h1;   // token q + 8
-          }
-          sa[c][mi][0] = __half2float(p.sA[static_cast<size_t>(gam[c]) * kTileRows + 16 * mi + q]);
-          sa[c][mi][1] = __half2float(p.sA[static_cast<size_t>(gam[c]) * kTileRows + 16 * mi + q + 8]);
+        for (int e = 0; e < 4; ++e) yf[i][mi][e] = 0.f;
+
+    for (int j = 0; j < nkw; ++j) {
+      const uint32_t st = my_stage0 + cslot * Cfg::kStageBytes;
+      mbar_wait(my_bar0 + 8 * cslot, (par >> cslot) & 1);
+      par ^= 1u << cslot;
+      // ---- token fragments of this k-block (widened once, reused by every row block)
+      uint32_t af[MT][4][4];
+      float sa[MT][2];
+#pragma unroll
+      for (int mi = 0; mi < MT; ++mi) {
+        uint32_t x0[4], x1[4];
+        lds128(st + Cfg::kWBytes + (16 * mi) * kRowBytes + lane_off, x0[0], x0[1], x0[2], x0[3]);
+        lds128(st + Cfg::kWBytes + (16 * mi + 8) * kRowBytes + lane_off, x1[0], x1[1], x1[2], x1[3]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const uint32_t l0 = rotl4(x0[i]) & kMask, h0 = x0[i] & kMask;
+          const uint32_t l1 = rotl4(x1[i]) & kMask, h1 = x1[i] & kMask;
+          af[mi][i][0] = swap ? h0 : l0; af[mi][i][2] = swap ? l0 : h0;   // token q: k lo / hi half
+          af[mi][i][1] = swap ? h1 : l1; af[mi][i][3] = swap ? l1 : h1;   // token q + 8
         }
+        const __half* sah = reinterpret_cast<const __half*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes);
+        sa[mi][0] = __half2float(sah[16 * mi + q]);
+        sa[mi][1] = __half2float(sah[16 * mi + q + 8]);
       }
-      // ---- stream the weights of (row block i, k-block c), c fastest, through the register ring:
-      // ring slot d always holds k-block d % CC (D is a multiple of CC)
-      static_assert(D % CC == 0, "ring depth");
-      uint4 wq[D];
-      uint32_t sq[D];
-      const uint8_t* wbase = p.qW + static_cast<size_t>(kc) * kBlobBytes + lane_off;
-      auto issue = [&](int buf, int i, int c) {         // c is static at every call site
-        const int row0 = (b0 + i) * 8;
-        wq[buf] = ldg_stream(wbase + static_cast<size_t>(row0 >> 7) * row_pitch + static_cast<size_t>(c) * kBlobBytes +
-                             (row0 & 127) * kRowBytes);
-        const int n0 = row0 + 2 * t;                    // columns 2t, 2t+1 of the accumulator fragment
-        sq[buf] = ldg_u32(p.sW + (static_cast<size_t>(n0 >> 7) * p.G + gam[c]) * kTileRows + (n0 & 127));
-      };
-      constexpr int RB = D / CC;                        // row blocks per ring revolution
+      const int gm = DUMP ? (kbw0 + j) / p.kbu : 0;
 #pragma unroll
-      for (int d = 0; d < D - 1; ++d)
-        if (d / CC < nb) issue(d, d / CC, d % CC);
-      for (int ib = 0; ib < nb; ib += RB) {
-#pragma unroll
-        for (int d = 0; d < D; ++d) {
-          const int i = ib + d / CC;                    // row block of the batch
-          const int c = d % CC;
-          if (i >= nb) break;
-          {                                             // prefetch the unit D - 1 ahead
-            const int dn = d + D - 1;
-            const int in = ib + dn / CC;
-            if (in < nb) issue(dn % D, in, dn % CC);
-          }
+      for (int i = 0; i < RBB; ++i) {
+        if (i < nb) {
+          uint32_t x[4];
+          lds128(st + i * 512 + lane_off, x[0], x[1], x[2], x[3]);
+          const __half2 sw2 = *reinterpret_cast<const __half2*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + i * 16 + 4 * t);
           int acc[MT][4];
 #pragma unroll
           for (int mi = 0; mi < MT; ++mi)
@@ -157,55 +198,41 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
             for (int e = 0; e < 4; ++e) acc[mi][e] = 0;
 #pragma unroll
           for (int k4 = 0; k4 < 4; ++k4) {
-            const uint32_t x = word(wq[d], k4);
-            const uint32_t b0w = rotl4(x) & kMask, b1w = x & kMask;
+            const uint32_t b0w = rotl4(x[k4]) & kMask, b1w = x[k4] & kMask;
 #pragma unroll
-            for (int mi = 0; mi < MT; ++mi) mma_s8(acc[mi], af[c][mi][k4], b0w, b1w);
+            for (int mi = 0; mi < MT; ++mi) mma_s8(acc[mi], af[mi][k4], b0w, b1w);
           }
           // this k-block's sums: INT32 -> FP32, x sW / 256, x sA (a5)
-          const __half2 sw2 = *reinterpret_cast<const __half2*>(&sq[d]);
           const float sw0 = __low2float(sw2) * 0.00390625f, sw1 = __high2float(sw2) * 0.00390625f;
 #pragma unroll
           for (int mi = 0; mi < MT; ++mi) {
-            const float s0 = sa[c][mi][0], s1 = sa[c][mi][1];
-            if (c == 0) {
-              yfr[mi][0] = __int2float_rn(acc[mi][0]) * sw0 * s0;
-              yfr[mi][1] = __int2float_rn(acc[mi][1]) * sw1 * s0;
-              yfr[mi][2] = __int2float_rn(acc[mi][2]) * sw0 * s1;
-              yfr[mi][3] = __int2float_rn(acc[mi][3]) * sw1 * s1;
-            } else {
-              yfr[mi][0] = fmaf(__int2float_rn(acc[mi][0]) * sw0, s0, yfr[mi][0]);
-              yfr[mi][1] = fmaf(__int2float_rn(acc[mi][1]) * sw1, s0, yfr[mi][1]);
-              yfr[mi][2] = fmaf(__int2float_rn(acc[mi][2]) * sw0, s1, yfr[mi][2]);
-              yfr[mi][3] = fmaf(__int2float_rn(acc[mi][3]) * sw1, s1, yfr[mi][3]);
-            }
+            yf[i][mi][0] = fmaf(__int2float_rn(acc[mi][0]) * sw0, sa[mi][0], yf[i][mi][0]);
+            yf[i][mi][1] = fmaf(__int2float_rn(acc[mi][1]) * sw1, sa[mi][0], yf[i][mi][1]);
+            yf[i][mi][2] = fmaf(__int2float_rn(acc[mi][2]) * sw0, sa[mi][1], yf[i][mi][2]);
+            yf[i][mi][3] = fmaf(__int2float_rn(acc[mi][3]) * sw1, sa[mi][1], yf[i][mi][3]);
             if constexpr (DUMP) {
 #pragma unroll
               for (int e = 0; e < 4; ++e) {
                 const int m = 16 * mi + q + 8 * (e >> 1), n = (b0 + i) * 8 + 2 * t + (e & 1);
                 if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1)   // P_out is zero-filled by the caller
-                  atomicAdd(p.P_out + (static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gam[c],
+                  atomicAdd(p.P_out + (static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gm,
                             acc[mi][e] >> 8);
               }
             }
           }
-          if (c == CC - 1) {                            // row block done for this pass: add to the warp's slot
-#pragma unroll
-            for (int mi = 0; mi < MT; ++mi) {
-              float4* sl = &slots[((i * kWarps + w) * MT + mi) * 32 + lane];
-              float4 v = *sl;
-              v.x += yfr[mi][0]; v.y += yfr[mi][1]; v.z += yfr[mi][2]; v.w += yfr[mi][3];
-              *sl = v;
-            }
-          }
         }
       }
-    };
-    int kc = kbw0;
-    for (; kc + C <= kbw1; kc += C) pass(kc, std::integral_constant<int, C>{});
-    for (; kc < kbw1; ++kc) pass(kc, std::integral_constant<int, 1>{});
+      __syncwarp();                                     // every lane is done reading the stage
+      if (lane == 0) issue_next();                      // re-arm it with the warp's next k-block
+      cslot = cslot + 1 == kStages ? 0 : cslot + 1;
+    }
 
-    // ---- a6 / a7: sum the 16 warps' partials of every row block of the batch, cast, store
+    // ---- a6 / a7: the 16 warps' partials of the batch meet in shared memory; cast, store
+#pragma unroll
+    for (int i = 0; i < RBB; ++i)
+#pragma unroll
+      for (int mi = 0; mi < MT; ++mi)
+        part[((i * kWarps + w) * MT + mi) * 32 + lane] = make_float4(yf[i][mi][0], yf[i][mi][1], yf[i][mi][2], yf[i][mi][3]);
     __syncthreads();
     if (p.Y != nullptr) {
       for (int i = w; i < nb; i += kWarps) {
@@ -214,8 +241,8 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
           float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
           for (int ww = 0; ww < kWarps; ++ww) {
-            const float4 x = slots[((i * kWarps + ww) * MT + mi) * 32 + lane];
-            v.x += x.x; v.y += x.y; v.z += x.z; v.w += x.w;
+            const float4 xx = part[((i * kWarps + ww) * MT + mi) * 32 + lane];
+            v.x += xx.x; v.y += xx.y; v.z += xx.z; v.w += xx.w;
           }
           const int n = (b0 + i) * 8 + 2 * t;
           const int m = 16 * mi + q;
@@ -238,33 +265,31 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <int MT, int C>
-static cudaError_t launch_gemv_mc(const GemmParams& p, bool dump, int grid, cudaStream_t st) {
-  const int smem = p.upt * kWarps * MT * 512;
+template <int MT>
+static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaStream_t st) {
+  constexpr int smem = GemvCfg<MT>::kSmemBytes;
   cudaError_t e;
   if (dump) {
-    auto kern = w4a4_gemv_kernel<MT, C, true>;
-    if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSlotBudget)) != cudaSuccess) return e;
+    auto kern = w4a4_gemv_kernel<MT, true>;
+    if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     kern<<<grid, kThreads, smem, st>>>(p);
   } else {
-    auto kern = w4a4_gemv_kernel<MT, C, false>;
-    if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSlotBudget)) != cudaSuccess) return e;
+    auto kern = w4a4_gemv_kernel<MT, false>;
+    if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     kern<<<grid, kThreads, smem, st>>>(p);
   }
   return cudaGetLastError();
 }
 
-// mt: m16 token tiles (1..4).  p.upt (row blocks per batch) must be <= gemv_max_batch(mt).
+// mt: m16 token tiles (1 or 2; apex4_gemv_ring.cu takes 3 and 4)
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st) {
   switch (mt) {
-    case 1: return launch_gemv_mc<1, 2>(p, dump, grid, st);
-    case 2: return launch_gemv_mc<2, 1>(p, dump, grid, st);
-    case 3: return launch_gemv_mc<3, 1>(p, dump, grid, st);
-    case 4: return launch_gemv_mc<4, 1>(p, dump, grid, st);
+    case 1: return launch_gemv_m<1>(p, dump, grid, st);
+    case 2: return launch_gemv_m<2>(p, dump, grid, st);
     default: return cudaErrorInvalidValue;
   }
 }
 
-int gemv_max_batch(int mt) { return kSlotBudget / (kWarps * mt * 512); }
+int gemv_max_batch(int mt) { return mt == 1 ? 7 : mt == 2 ? 4 : mt == 3 ? 2 : 1; }
 
 }  // namespace apex4
