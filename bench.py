@@ -156,7 +156,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="apex4")
-    ap.add_argument("--sweep", action="store_true", help="also time the config-2 M sweep + cuBLAS FP16")
+    ap.add_argument("--sweep", action="store_true",
+                    help="also time the config-2 M sweep, config-3 granularities and config-4 decode shapes + cuBLAS FP16")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl != "reference":
@@ -276,7 +277,7 @@ def main():
     if os.path.exists(tp):
         traffic = json.load(open(tp)).get("gemm_dram_bytes_per_launch")
     roofline = {
-        "kernel": "w4a4_gemm_kernel<256> (tcgen05 kind::i8)", "bound": "tensor", "achieved": gemm_tops,
+        "kernel": "w4a4_gemm_pair_kernel (tcgen05 cta_group::2 kind::i8, 256x192 tiles)", "bound": "tensor", "achieved": gemm_tops,
         "peak": int8_peak, "unit": "TOP/s", "frac": gemm_tops / int8_peak, "traffic": traffic,
         "peak_source": f"2 x {peaks['bf16_sus']} sustained bf16 TFLOP/s of {peaks['src']} MEASURED_PEAKS.json "
                        "(nominal int8:bf16 ratio 4.5:2.25)",
@@ -307,7 +308,7 @@ def main():
                                          f"({secs:.1f} s of numpy float64 oracle)"}
     if args.sweep and rank == 0:
         from paper_2606_08761_b200 import sweep
-        out["sweep"] = sweep.run_sweeps(dev)
+        out["sweep"] = sweep.run_sweeps(dev, {"hbm": peaks["hbm"], "int8": int8_peak})
     if rank == 0:
         print(json.dumps(out))
     if world > 1:

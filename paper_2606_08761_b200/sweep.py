@@ -1,0 +1,107 @@
+"""Shape sweeps behind `bench.py --sweep`: BASELINE.json config 2 (N = K = 8192, g = 128,
+M from decode to prefill), config 3 (granularities at M = 4096) and the decode rows of config 4
+(Llama-2-70B linears at M = 1, 16).  Per shape: GEMM time, effective TOPS (2MNK/t), the fraction of
+the roofline that binds (INT8 tensor peak for M >= 256, HBM copy bandwidth below), and the speed-up
+over cuBLAS FP16 (`torch.matmul`) on the same (M, N, K).
+
+Timing protocol: every shape is captured in a CUDA graph of 20 launches that rotate through operand
+sets whose total size exceeds L2 (so weights come from HBM), replayed 10 times, median reported;
+CUDA events on the launching stream.  Operands are random packed codes / scales of the right
+layouts (timing does not depend on the values); parity is the business of tests/.
+"""
+from __future__ import annotations
+
+import torch
+
+from . import apex4
+
+L2_BYTES = 126e6
+GRAPH_LAUNCHES = 20
+
+
+def _graph_time_us(fn, nsets: int) -> float:
+    for i in range(max(nsets, 3)):
+        fn(i % nsets)
+    torch.cuda.synchronize()
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr):
+        for i in range(GRAPH_LAUNCHES):
+            fn(i % nsets)
+    ts = []
+    for _ in range(10):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        gr.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) / GRAPH_LAUNCHES * 1e3)
+    ts.sort()
+    return ts[len(ts) // 2]
+
+
+def gemm_bytes(M, N, K, g):
+    """Algorithmic bytes of one GEMM: packed codes, FP16 scales, FP16 output."""
+    G = K // g
+    return N * K / 2 + 2 * N * G + M * K / 2 + 2 * M * G + 2 * M * N
+
+
+def time_shape(M, N, K, g, dev, cublas=True):
+    per_set = N * K / 2 + M * K / 2
+    nsets = int(max(1, min(8, 2 * L2_BYTES // per_set + 1)))
+    sets = []
+    for _ in range(nsets):
+        qA = torch.randint(0, 256, (apex4.packed_bytes(M, K),), dtype=torch.uint8, device=dev)
+        qW = torch.randint(0, 256, (apex4.packed_bytes(N, K),), dtype=torch.uint8, device=dev)
+        sA = (torch.rand(apex4.scale_elems(M, K, g), device=dev) * 0.1 + 0.01).half()
+        sW = (torch.rand(apex4.scale_elems(N, K, g), device=dev) * 0.01 + 0.001).half()
+        sets.append((qA, sA, qW, sW))
+    Y = torch.empty((M, N), dtype=torch.float16, device=dev)
+    ws = apex4.make_workspace(M, N, K, g, device=dev)
+
+    def run(i):
+        qA, sA, qW, sW = sets[i]
+        apex4.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out=Y, workspace=ws)
+
+    us = _graph_time_us(run, nsets)
+    out = {"M": M, "N": N, "K": K, "g": g, "us": round(us, 2),
+           "tops": round(2.0 * M * N * K / us * 1e-6, 1),
+           "gbs": round(gemm_bytes(M, N, K, g) / us * 1e-3, 1),
+           "kernel": {0: "gemv", 256: "pair"}.get(apex4.debug_get_dispatch(M, N, K, g)[0], "tile")}
+    del sets
+    if cublas:
+        nb = int(max(1, min(4, 2 * L2_BYTES // (2 * N * K) + 1)))
+        a = torch.randn(M, K, device=dev, dtype=torch.float16)
+        bs = [torch.randn(N, K, device=dev, dtype=torch.float16) for _ in range(nb)]
+        c = torch.empty((M, N), device=dev, dtype=torch.float16)
+        cu = _graph_time_us(lambda i: torch.matmul(a, bs[i].t(), out=c), nb)
+        out["cublas_fp16_us"] = round(cu, 2)
+        out["speedup_vs_cublas_fp16"] = round(cu / us, 2)
+        del bs
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_sweeps(dev, peaks=None):
+    """-> dict of lists; `peaks` = {"hbm": GB/s, "int8": TOP/s} adds the roofline fractions."""
+    res = {"protocol": f"CUDA graph of {GRAPH_LAUNCHES} launches rotating operand sets larger than L2, median of 10 replays"}
+    cfg2 = [time_shape(M, 8192, 8192, 128, dev) for M in (1, 4, 16, 64, 256, 1024, 4096, 8192)]
+    cfg3 = [time_shape(4096, 8192, 8192, g, dev, cublas=False) for g in (32, 64, 128, 8192)]
+    cfg4 = [time_shape(M, N, K, 128, dev) for (N, K) in ((10240, 8192), (8192, 8192), (57344, 8192), (8192, 28672))
+            for M in (1, 16)]
+    if peaks:
+        for r in cfg2 + cfg3 + cfg4:
+            if r["M"] >= 256:
+                r["bound"] = "tensor"
+                r["frac_of_int8_peak"] = round(r["tops"] / peaks["int8"], 3)
+            else:
+                r["bound"] = "hbm"
+                r["frac_of_hbm_peak"] = round(r["gbs"] / peaks["hbm"], 3)
+    res["config2_square_sweep"] = cfg2
+    res["config3_granularity"] = cfg3
+    t = {r["g"]: r["us"] for r in cfg3}
+    res["config3_mixed"] = {   # R11: 2 fine layers (V, DOWN) + 5 per-channel layers per block, mapped on this shape
+        "paper_mix_fine32_us": round((2 * t[32] + 5 * t[8192]) / 7, 2),
+        "baseline_mix_fine128_us": round((2 * t[128] + 5 * t[8192]) / 7, 2),
+        "uniform_g128_us": t[128]}
+    res["config4_decode"] = cfg4
+    return res
