@@ -77,13 +77,20 @@ def test_argument_validation_without_gpu(L):
 def test_dispatch_table(L):
     """Host-side choice of token-tile width / work distribution (a6, a8): pure host code."""
     from paper_2606_08761_b200 import apex4
+    # decode regime, g = 128: the streaming kernel (nt = 0), 8-row row blocks over all SMs, no workspace
     nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 128)
-    assert (nt, split, upt) == (16, 1, 64) and 1 <= grid <= 148     # decode: stream-K over all SMs
+    assert (nt, split, upt) == (0, 0, 7) and 1 <= grid <= 148
+    assert apex4.debug_get_dispatch(64, 8192, 8192, 128)[0] == 0
+    assert apex4.workspace_bytes(16, 8192, 8192, 128) == 0
+    # tensor-bound regime: CTA pairs on 256 x 192 tiles; 43 x 32 tiles fill the last wave -> whole tiles
     nt, split, grid, upt = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
-    assert (nt, split, upt) == (256, 0, 64)                          # 2048 tiles: whole tiles per CTA
-    # per-channel: the k range cannot be split inside a group
+    assert (nt, split, upt) == (256, 0, 64) and 1 <= grid <= 74
+    assert apex4.workspace_bytes(8192, 8192, 8192, 128) == 0
+    # Llama-2-7B O-proj at M = 2048: 11 x 16 tiles on <= 74 pairs -> stream-K with the FP32 workspace
+    nt, split, grid, upt = apex4.debug_get_dispatch(2048, 4096, 4096, 128)
+    assert (nt, split, upt) == (256, 1, 32)
+    assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 2048 * 4096 * 4    # 11 * 16 * 2 counters, padded
+    # per-channel at small M: the tile kernel; the k range cannot be split inside a group
     nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
     assert (nt, split, grid, upt) == (16, 0, 64, 1)
-    assert apex4.workspace_bytes(8192, 8192, 8192, 128) == 0
     assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0
-    assert apex4.workspace_bytes(16, 8192, 8192, 128) == 256 + 16 * 8192 * 4

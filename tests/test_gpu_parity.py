@@ -163,6 +163,24 @@ def test_gemm_ragged_and_multi_tile(A, M, N, K, g):
     run_gemm_case(A, M, N, K, g, seed=100 + M)
 
 
+@pytest.mark.parametrize("M,N,K", [(1, 8, 128), (16, 136, 1024), (17, 1000, 512), (32, 8192, 256),
+                                   (33, 264, 2048), (48, 520, 1024), (64, 456, 1536), (5, 64, 28672)])
+@pytest.mark.parametrize("grid", [-1, 1, 3])
+def test_gemm_decode_kernels(A, M, N, K, grid):
+    """The decode-regime kernels (M <= 64, g = 128: bulk-copy staged for one or two m16 token tiles,
+    register-ring for three or four) on ragged N, row ranges that straddle 128-row tiles, K from one
+    k-block to the longest supported row, and several grid sizes (rows per CTA / batches per CTA)."""
+    assert A.debug_get_dispatch(M, N, K, 128)[0] == 0          # automatic dispatch picks the decode kernel
+    run_gemm_case(A, M, N, K, 128, seed=300 + M, dispatch=(0, -1, grid))
+
+
+def test_gemm_decode_f32_and_large_group_routing(A):
+    run_gemm_case(A, 16, 256, 1024, 128, seed=7, out_f32=True, dispatch=(0, -1, -1))
+    # groups larger than a k-block keep one rounding per group: the tile kernel handles them
+    assert A.debug_get_dispatch(16, 256, 1024, 256)[0] != 0
+    run_gemm_case(A, 16, 256, 1024, 256, seed=8)
+
+
 def test_gemm_f32_output(A):
     run_gemm_case(A, 40, 256, 1024, 128, seed=3, out_f32=True)
     run_gemm_case(A, 200, 512, 1024, 128, seed=4, out_f32=True)
