@@ -130,7 +130,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
                 bScfEmpty = bScfFull + kScfSlots, bAccFull = bScfEmpty + kScfSlots,
                 bAccEmpty = bAccFull + kAccBufs;
 
-  const int warp = threadIdx.x >> 5;
+  // warp index through a shuffle from lane 0: tells the compiler it is warp-uniform, so addresses derived
+  // from it (TMEM lane quarter, barrier and stage addresses) live in uniform registers (no R2UR per use)
+  const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
   const int lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();      // 0 = leader
   const int cp = blockIdx.x >> 1;               // pair index
@@ -422,6 +424,12 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
     const int epi_tid = threadIdx.x - 32 * kEpiWarp0;
     const uint32_t lane_addr = static_cast<uint32_t>(lq * 32) << 16;
     const int row0 = lq * 32 + q;                       // rows row0 + 8 i, i = 0..3
+    // per-thread address parts of the group loop, made opaque so that ptxas keeps them in registers
+    // instead of re-deriving them from %tid in every group (11 S2R + ~40 integer ops per group)
+    uint32_t tm_rd = lane_addr + h * kHalf;                                   // + buf * kNT
+    uint32_t ab_off = offScf + row0 * 8;                                      // {a, b} of row row0 (+ 64 i)
+    uint32_t sa_off = offScf + kTileRows * 8 + (h * kHalf) * 4 + t * 16;      // token scales (+ 64 c)
+    asm volatile("" : "+r"(tm_rd), "+r"(ab_off), "+r"(sa_off));
     // the magic bias in 8 registers, read through a volatile load so that ptxas keeps them resident
     // instead of re-materialising 16 constants per tcgen05.st (IMAD.MOV on the FMA pipe)
     uint32_t mg[8];
@@ -458,20 +466,20 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
         const int slot = gc % kScfSlots;
         const uint32_t buf = gc & 1;
         mbar_wait(bar(bScfFull + slot), (gc / kScfSlots) & 1);
-        const uint32_t scf = smem_base + offScf + slot * kScfSlotBytes;
+        const uint32_t scf = smem_base + slot * kScfSlotBytes;
         uint64_t a2[4], b2[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           float af, bf;
-          unpack_f2(lds64(scf + (row0 + 8 * i) * 8), af, bf);
+          unpack_f2(lds64(scf + ab_off + 64 * i), af, bf);
           a2[i] = pack_f2(af, af);
           b2[i] = pack_f2(bf, bf);
         }
-        const uint32_t sAf = scf + kTileRows * 8 + (h * kHalf) * 4 + t * 16;   // + 64 c
+        const uint32_t sAf = scf + sa_off;   // + 64 c
         mbar_wait(bar(bAccFull + buf), (gc >> 1) & 1);
         tc_fence_after();
         if (epi_tid == 0) stamp(6, gc);
-        const uint32_t tb = tmem_base + lane_addr + buf * kNT + h * kHalf;
+        const uint32_t tb = tm_rd + buf * kNT;
         uint32_t v[2][16];
         uint64_t sq[2][2];                               // token scales of chunk c, c + 1
         lds_2x64(sAf, sq[0][0], sq[0][1]);
