@@ -140,6 +140,14 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
   const int g = p.g;
   const int gpk = g < kBlockK ? kBlockK / g : 1;        // groups per k-block (1, 2, 4)
   const int kbpg = g > kBlockK ? g / kBlockK : 1;       // k-blocks per group
+  // Scale-slot hand-shake.  At g = 128 (one group per k-block) it is implied by the operand / accumulator
+  // barriers and skipped -- every mbarrier wait costs ~250 clk even when the phase is already complete:
+  //  * full:  the wideners write slot k before they publish operand stage k, the MMA of group k is
+  //           issued after that, so "accumulator k full" implies "scales k written";
+  //  * empty: the widener of k-block k has waited for operand stage k % 4 = MMA k-4 done, which was
+  //           issued after all epilogue warps released accumulator k-6, i.e. had finished group k-8,
+  //           the previous user of slot k % 8.
+  const bool scf_sync = g != kBlockK;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kPkStages; ++i) { mbar_init(bar(bPkFull + i), 1); mbar_init(bar(bPkEmpty + i), 128); }
@@ -373,24 +381,15 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
             }
           }
         }
-        // ---- publish stage t: one elected arrive per warp on the leader's barrier
-        if (r == 0) stamp(10, kbc);
-        fence_proxy_async_smem();
-        if (r == 0) stamp(11, kbc);
-        tmem_st_wait();
-        if (r == 0) stamp(12, kbc);
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(bar(bOpFull + t_cur), 0);
-        if (r == 0) stamp(3, kbc);
-        // ---- scales of the groups that start in this k-block: FP16 -> FP32
+        // ---- scales of the groups that start in this k-block: FP16 -> FP32, BEFORE the stage is published:
+        // at g = 128 the epilogue takes "accumulator full" as "scales written" (see scf_sync)
         if (starts_group) {
           const uint8_t* pk = smem_gen + offPk + s_cur * kPkStageBytes;
           const __half* sWh = reinterpret_cast<const __half*>(pk + kPkWBytes + kPkABytes);
           const __half* sAh = sWh + kPkSWBytes / 2;     // [blob 0/1][sub][128]
           for (int sub = 0; sub < gpk; ++sub, ++gc) {
             const int q = gc % kScfSlots;
-            mbar_wait(bar(bScfEmpty + q), ((gc / kScfSlots) & 1) ^ 1);
+            if (scf_sync) mbar_wait(bar(bScfEmpty + q), ((gc / kScfSlots) & 1) ^ 1);
             float* dstf = reinterpret_cast<float*>(smem_gen + offScf + q * kScfSlotBytes);
             const float sw = __half2float(sWh[sub * kTileRows + r]);
             // a = sW / 256 (the operands are 16 q each); b = -12582912 * a removes the magic bias
@@ -407,9 +406,19 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
                 dstf[2 * kTileRows + pos] = __half2float(sAh[((mm >> 7) * gpk + sub) * kTileRows + (mm & 127)]);
               }
             }
-            mbar_arrive(bar(bScfFull + q));
+            if (scf_sync) mbar_arrive(bar(bScfFull + q));
           }
         }
+        // ---- publish stage t: one elected arrive per warp on the leader's barrier
+        if (r == 0) stamp(10, kbc);
+        fence_proxy_async_smem();
+        if (r == 0) stamp(11, kbc);
+        tmem_st_wait();
+        if (r == 0) stamp(12, kbc);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(bar(bOpFull + t_cur), 0);
+        if (r == 0) stamp(3, kbc);
         mbar_arrive(bar(bPkEmpty + s_cur));
         if (r == 0) stamp(13, kbc);
       }
@@ -465,7 +474,8 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       for (int gi = 0; gi < ngroups; ++gi, ++gc) {
         const int slot = gc % kScfSlots;
         const uint32_t buf = gc & 1;
-        mbar_wait(bar(bScfFull + slot), (gc / kScfSlots) & 1);
+        if (scf_sync) mbar_wait(bar(bScfFull + slot), (gc / kScfSlots) & 1);
+        mbar_wait(bar(bAccFull + buf), (gc >> 1) & 1);
         const uint32_t scf = smem_base + slot * kScfSlotBytes;
         uint64_t a2[4], b2[4];
 #pragma unroll
@@ -476,7 +486,6 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
           b2[i] = pack_f2(bf, bf);
         }
         const uint32_t sAf = scf + sa_off;   // + 64 c
-        mbar_wait(bar(bAccFull + buf), (gc >> 1) & 1);
         tc_fence_after();
         if (epi_tid == 0) stamp(6, gc);
         const uint32_t tb = tm_rd + buf * kNT;
@@ -537,8 +546,10 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
             acc[(i * kChunks + c) * 2 + 1] = fma2(t1, s23, acc[(i * kChunks + c) * 2 + 1]);
           }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar(bScfEmpty + slot));
+        if (scf_sync) {
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar(bScfEmpty + slot));
+        }
         if (epi_tid == 0) stamp(7, gc);
       }
 
