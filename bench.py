@@ -309,6 +309,7 @@ def main():
     if args.sweep and rank == 0:
         from paper_2606_08761_b200 import sweep
         out["sweep"] = sweep.run_sweeps(dev, {"hbm": peaks["hbm"], "int8": int8_peak})
+        out["rho"] = apex4.measure_rho()      # B200's own rho: INT8 tensor ops vs FP32 FMA (Table 1)
     if rank == 0:
         print(json.dumps(out))
     if world > 1:
