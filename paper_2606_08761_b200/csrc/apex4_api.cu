@@ -136,7 +136,10 @@ cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, c
   return e;
 }
 size_t workspace_need(const Dispatch& d, int M, int N) {
-  return d.split ? counters_bytes(d) + static_cast<size_t>(M) * N * 4 : 0;
+  if (!d.split) return 0;
+  // pair kernel: every 256 x 192 tile in fragment order (tile-padded); tile kernel: [M, N]
+  if (d.nt == 256) return counters_bytes(d) + static_cast<size_t>(d.tiles_m) * d.tiles_n * 256 * kPairTokens * 4;
+  return counters_bytes(d) + static_cast<size_t>(M) * N * 4;
 }
 
 int validate_gemm_shape(int M, int N, int K) {

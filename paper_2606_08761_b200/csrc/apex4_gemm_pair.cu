@@ -556,7 +556,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       // ---- a7 (cast + store) or a6 (cross-pair reduce through the FP32 workspace)
       if (epi_tid == 0) stamp(15, item * 4 + 1);
       if (p.Y != nullptr) {
-        if (!w.partial) {
+        auto store_tile = [&]() {
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int n = n_glob0 + 8 * i;
@@ -579,24 +579,25 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
                 }
               }
           }
+        };
+        if (!w.partial) {
+          store_tile();
         } else {
-          // a6: FP32 partial sums meet in the workspace (red.add at L2); the CTA that completes its
-          // half of the tile casts, stores and leaves the workspace zero-filled again (PAPER.md:230
-          // "inter-SM global reduction").
+          // a6: FP32 partial sums meet in the workspace ("inter-SM global reduction").  The
+          // workspace holds every CTA tile in FRAGMENT order -- [tile][CTA][j = 0..23][thread][4 floats] --
+          // so a partial tile is 24 fully coalesced red.global.add.v4.f32 per thread (not 96 scalar
+          // atomics), and the CTA that completes the tile reads it back with the same thread mapping,
+          // leaves it zero-filled, casts and stores.
+          float* wst = p.ws + static_cast<size_t>((w.nt * p.tiles_m + w.mt) * 2 + static_cast<int>(rank)) * (kTileRows * kNT) +
+                       epi_tid * 4;
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int n = n_glob0 + 8 * i;
-            if (n >= p.N) continue;
-#pragma unroll
-            for (int c = 0; c < kChunks; ++c)
-#pragma unroll
-              for (int j = 0; j < 2; ++j) {
-                float f0, f1;
-                unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
-                const int m = m_glob0 + 16 * c + 8 * j;
-                if (m < p.M) atomicAdd(p.ws + static_cast<size_t>(m) * p.N + n, f0);
-                if (m + 1 < p.M) atomicAdd(p.ws + static_cast<size_t>(m + 1) * p.N + n, f1);
-              }
+          for (int j = 0; j < 4 * kChunks; ++j) {
+            float f0, f1, f2, f3;
+            unpack_f2(acc[2 * j], f0, f1);
+            unpack_f2(acc[2 * j + 1], f2, f3);
+            asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(wst + j * 1024), "f"(f0),
+                         "f"(f1), "f"(f2), "f"(f3)
+                         : "memory");
           }
           __threadfence();
           if (epi_tid == 0) stamp(15, item * 4 + 2);
@@ -613,41 +614,16 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
           const int done = *flag;
           asm volatile("bar.sync 1, 256;" ::: "memory");   // flag may be rewritten by the next item
           if (done) {
-            // all loads first (the running sums are dead: their registers hold the tile), then the
-            // stores -- a load/store/load chain here costs one L2 round trip per element
             __threadfence();
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const int n = n_glob0 + 8 * i;
-#pragma unroll
-              for (int cj = 0; cj < 2 * kChunks; ++cj) {
-                const int m = m_glob0 + 8 * cj;
-                float f0 = 0.f, f1 = 0.f;
-                if (n < p.N && m < p.M) f0 = __ldcg(p.ws + static_cast<size_t>(m) * p.N + n);
-                if (n < p.N && m + 1 < p.M) f1 = __ldcg(p.ws + static_cast<size_t>(m + 1) * p.N + n);
-                acc[i * 2 * kChunks + cj] = pack_f2(f0, f1);
-              }
+            for (int j = 0; j < 4 * kChunks; ++j) {       // all loads first, then the zero stores
+              const float4 x = __ldcg(reinterpret_cast<const float4*>(wst + j * 1024));
+              acc[2 * j] = pack_f2(x.x, x.y);
+              acc[2 * j + 1] = pack_f2(x.z, x.w);
             }
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const int n = n_glob0 + 8 * i;
-              if (n >= p.N) continue;
-#pragma unroll
-              for (int cj = 0; cj < 2 * kChunks; ++cj) {
-                float f[2];
-                unpack_f2(acc[i * 2 * kChunks + cj], f[0], f[1]);
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  const int m = m_glob0 + 8 * cj + e;
-                  if (m < p.M) {
-                    const size_t idx = static_cast<size_t>(m) * p.N + n;
-                    __stcg(p.ws + idx, 0.f);
-                    if (p.out_f32) static_cast<float*>(p.Y)[idx] = f[e];
-                    else static_cast<__half*>(p.Y)[idx] = __float2half_rn(f[e]);
-                  }
-                }
-              }
-            }
+            for (int j = 0; j < 4 * kChunks; ++j) __stcg(reinterpret_cast<float4*>(wst + j * 1024), make_float4(0.f, 0.f, 0.f, 0.f));
+            store_tile();
           }
         }
       }

@@ -89,7 +89,8 @@ def test_dispatch_table(L):
     # Llama-2-7B O-proj at M = 2048: 11 x 16 tiles on <= 74 pairs -> stream-K with the FP32 workspace
     nt, split, grid, upt = apex4.debug_get_dispatch(2048, 4096, 4096, 128)
     assert (nt, split, upt) == (256, 1, 32)
-    assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 2048 * 4096 * 4    # 11 * 16 * 2 counters, padded
+    # 11 * 16 * 2 counters (padded to 256 bytes) + every 256 x 192 tile as FP32 in fragment order
+    assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 11 * 16 * 256 * 192 * 4
     # per-channel at small M: the tile kernel; the k range cannot be split inside a group
     nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
     assert (nt, split, grid, upt) == (16, 0, 64, 1)
