@@ -88,8 +88,7 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
   else if (M <= 16) d.nt = 16;
   else if (M <= 32) d.nt = 32;
   else if (M <= 64) d.nt = 64;
-  else if (M <= 128) d.nt = 128;
-  else d.nt = 256;
+  else d.nt = 256;   // the pair kernel also wins for 64 < M <= 128 (40.7 vs 44.0 us at N = K = 8192); nt = 128 only when forced
   if (d.nt == 0) {
     // decode kernel: a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
     d.bias = 0;
@@ -117,7 +116,9 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
   // whole tiles per CTA when the last wave is reasonably full, stream-K otherwise
   const long long waves = (tiles + d.grid - 1) / d.grid;
   const double eff = static_cast<double>(tiles) / static_cast<double>(waves * d.grid);
-  d.split = (g_force_split >= 0) ? g_force_split : (eff < 0.93 ? 1 : 0);
+  // a single, reasonably full wave is cheaper as whole tiles than as stream-K ranges (each partial range
+  // pays a reduction and a pipeline restart: M = 256, N = K = 8192 57.7 us whole vs 61.5 us split)
+  d.split = (g_force_split >= 0) ? g_force_split : ((eff < 0.93 && !(waves == 1 && eff >= 0.8)) ? 1 : 0);
   if (d.upt == 1) d.split = 0;                      // nothing to split
   if (!d.split && tiles < d.grid) d.grid = static_cast<int>(tiles);
   return d;
