@@ -1,15 +1,18 @@
 """Shape sweeps behind `bench.py --sweep`: BASELINE.json config 2 (N = K = 8192, g = 128,
-M from decode to prefill), config 3 (granularities at M = 4096) and the decode rows of config 4
-(Llama-2-70B linears at M = 1, 16).  Per shape: GEMM time, effective TOPS (2MNK/t), the fraction of
+M from decode to prefill), config 3 (granularities at M = 4096) and config 4 (Llama-2-70B linears at
+M = 1, 16, 256, 4096).  Per shape: GEMM time, effective TOPS (2MNK/t), the fraction of
 the roofline that binds (INT8 tensor peak for M >= 256, HBM copy bandwidth below), and the speed-up
 over cuBLAS FP16 (`torch.matmul`) on the same (M, N, K).
 
 Timing protocol: every shape is captured in a CUDA graph of 20 launches that rotate through operand
 sets whose total size exceeds L2 (so weights come from HBM), replayed 10 times, median reported;
+shapes run in order of increasing work with an idle gap before each (see run_sweeps);
 CUDA events on the launching stream.  Operands are random packed codes / scales of the right
 layouts (timing does not depend on the values); parity is the business of tests/.
 """
 from __future__ import annotations
+
+import time
 
 import torch
 
@@ -84,10 +87,22 @@ def time_shape(M, N, K, g, dev, cublas=True):
 def run_sweeps(dev, peaks=None):
     """-> dict of lists; `peaks` = {"hbm": GB/s, "int8": TOP/s} adds the roofline fractions."""
     res = {"protocol": f"CUDA graph of {GRAPH_LAUNCHES} launches rotating operand sets larger than L2, median of 10 replays"}
-    cfg2 = [time_shape(M, 8192, 8192, 128, dev) for M in (1, 4, 16, 64, 256, 1024, 4096, 8192)]
-    cfg3 = [time_shape(4096, 8192, 8192, g, dev, cublas=False) for g in (32, 64, 128, 8192)]
-    cfg4 = [time_shape(M, N, K, 128, dev) for (N, K) in ((10240, 8192), (8192, 8192), (57344, 8192), (8192, 28672))
-            for M in (1, 16)]
+    # All shapes are timed in order of increasing work, each after a short idle gap: right after seconds
+    # of tensor-bound work the part is still under its power cap, and a shape timed then ran up to 45 %
+    # slower (M = 16, N = K = 8192: 16.2 vs 11.2 us; M = 256, N = 8192, K = 28672: 335 vs 180 us).
+    shapes70 = ((10240, 8192), (8192, 8192), (57344, 8192), (8192, 28672))
+    jobs = [("cfg2", M, 8192, 8192, 128, True) for M in (1, 4, 16, 64, 256, 1024, 4096, 8192)]
+    jobs += [("cfg3", 4096, 8192, 8192, g, False) for g in (32, 64, 128, 8192)]
+    jobs += [("cfg4", M, N, K, 128, True) for M in (1, 16, 256, 4096) for (N, K) in shapes70]
+    done = {}
+    for i in sorted(range(len(jobs)), key=lambda i: jobs[i][1] * jobs[i][2] * jobs[i][3]):
+        tag, M, N, K, g, cub = jobs[i]
+        torch.cuda.synchronize()
+        time.sleep(0.5)
+        done[i] = time_shape(M, N, K, g, dev, cublas=cub)
+    cfg2 = [done[i] for i in range(len(jobs)) if jobs[i][0] == "cfg2"]
+    cfg3 = [done[i] for i in range(len(jobs)) if jobs[i][0] == "cfg3"]
+    cfg4 = [done[i] for i in range(len(jobs)) if jobs[i][0] == "cfg4"]
     if peaks:
         for r in cfg2 + cfg3 + cfg4:
             if r["M"] >= 256:
@@ -103,5 +118,5 @@ def run_sweeps(dev, peaks=None):
         "paper_mix_fine32_us": round((2 * t[32] + 5 * t[8192]) / 7, 2),
         "baseline_mix_fine128_us": round((2 * t[128] + 5 * t[8192]) / 7, 2),
         "uniform_g128_us": t[128]}
-    res["config4_decode"] = cfg4
+    res["config4_llama70b"] = cfg4
     return res
