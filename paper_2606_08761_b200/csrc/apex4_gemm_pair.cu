@@ -61,8 +61,9 @@ constexpr int kI8StageBytes = kHalf * kBlockK;    // widened tokens: [96 rows][1
 constexpr int kScfSlotBytes = kTileRows * 8 + kNT * 4 + 256;   // {a,b} per row, sA per column (padded)
 constexpr int kRegsCtl = 32, kRegsWiden = 40, kRegsEpi = 184;  // launch: 96 per thread
 constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs;
+constexpr int kStoreBytes = kHalf * 64;            // per epilogue warp: [96 m][32 n] FP16 output staging
 constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
-                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64;
+                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + 8 * kStoreBytes;
 static_assert((kWidenWGs & (kWidenWGs - 1)) == 0 && (kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
 static_assert((kOpStages & (kOpStages - 1)) == 0, "stage index wraps with a mask");
 static_assert(kAccBufs * kNT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
@@ -124,6 +125,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
   constexpr uint32_t offBar = offScf + kScfSlots * kScfSlotBytes;
   constexpr uint32_t offTmemPtr = offBar + kNumBars * 8;
   constexpr uint32_t offMagic = offTmemPtr + 64;       // 8 words of the magic bias (see epilogue)
+  constexpr uint32_t offStore = (offMagic + 64 + 15) / 16 * 16;   // 8 x kStoreBytes output staging
   auto bar = [&](int i) { return smem_base + offBar + 8u * i; };
   constexpr int bPkFull = 0, bPkEmpty = bPkFull + kPkStages, bOpFull = bPkEmpty + kPkStages,
                 bOpEmpty = bOpFull + kOpStages, bScfFull = bOpEmpty + kOpStages,
@@ -557,6 +559,40 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       if (epi_tid == 0) stamp(15, item * 4 + 1);
       if (p.Y != nullptr) {
         auto store_tile = [&]() {
+          if (!p.out_f32) {
+            // FP16 output: the warp's 32 (n) x 96 (m) sub-tile is transposed through a private 6 KB
+            // shared-memory tile [m][32 n] (16-byte part p of row m stored at p ^ ((m >> 1) & 3): both the
+            // 2-byte scatter and the 16-byte gather are bank-conflict free), then written as 16-byte
+            // row pieces: 12 STG.128 per thread instead of 96 STG.U16 with 64-bit address arithmetic
+            // (the store phase was 10-12 % of the config-1 GEMM time)
+            const uint32_t stg = smem_base + offStore + (warp - kEpiWarp0) * kStoreBytes;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+              for (int c = 0; c < kChunks; ++c)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                  float f0, f1;
+                  unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
+                  const uint32_t a0 = stg + (16 * c + 8 * j + 2 * t) * 64 + ((i ^ t) << 4) + 2 * q;   // row m, column n = q + 8 i
+                  asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0), "h"(__half_as_ushort(__float2half_rn(f0))) : "memory");
+                  asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0 + 64), "h"(__half_as_ushort(__float2half_rn(f1))) : "memory");
+                }
+            __syncwarp();
+            const int n = (2 * w.nt + static_cast<int>(rank)) * kTileRows + lq * 32 + (lane & 3) * 8;
+            __half* ybase = static_cast<__half*>(p.Y) + n;
+#pragma unroll
+            for (int ps = 0; ps < kHalf / 8; ++ps) {
+              const int row = ps * 8 + (lane >> 2);
+              uint32_t x0, x1, x2, x3;
+              lds128(stg + row * 64 + (((lane & 3) ^ ((row >> 1) & 3)) << 4), x0, x1, x2, x3);
+              const int m = w.mt * kNT + h * kHalf + row;
+              if (m < p.M && n < p.N)
+                *reinterpret_cast<uint4*>(ybase + static_cast<size_t>(m) * p.N) = make_uint4(x0, x1, x2, x3);
+            }
+            __syncwarp();
+            return;
+          }
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int n = n_glob0 + 8 * i;
@@ -568,15 +604,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
                 float f0, f1;
                 unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
                 const int m = m_glob0 + 16 * c + 8 * j;
-                if (p.out_f32) {
-                  float* y = static_cast<float*>(p.Y);
-                  if (m < p.M) y[static_cast<size_t>(m) * p.N + n] = f0;
-                  if (m + 1 < p.M) y[static_cast<size_t>(m + 1) * p.N + n] = f1;
-                } else {
-                  __half* y = static_cast<__half*>(p.Y);
-                  if (m < p.M) y[static_cast<size_t>(m) * p.N + n] = __float2half_rn(f0);
-                  if (m + 1 < p.M) y[static_cast<size_t>(m + 1) * p.N + n] = __float2half_rn(f1);
-                }
+                float* y = static_cast<float*>(p.Y);
+                if (m < p.M) y[static_cast<size_t>(m) * p.N + n] = f0;
+                if (m + 1 < p.M) y[static_cast<size_t>(m + 1) * p.N + n] = f1;
               }
           }
         };
