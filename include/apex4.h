@@ -82,8 +82,12 @@ int apex4_resolve_group_size(int K, int group_size, int gran, int layer);
 size_t apex4_packed_bytes(int R, int K);
 /* Number of FP16 elements of the ST16 scale buffer for R rows at resolved group size g. */
 size_t apex4_scale_elems(int R, int K, int g);
-/* Bytes of workspace apex4_w4a4_gemm needs for this problem (0 if none).  The workspace must be
- * zero-filled once by the caller before its first use; every call leaves it zero-filled again. */
+/* Bytes of DEVICE workspace apex4_w4a4_gemm needs for this problem.  0 when every output tile is
+ * computed by one CTA (pair) alone: the decode kernels (M <= 64 at g = 128) and any tile count that
+ * fills the SMs evenly.  Otherwise (stream-K, a6) it holds the tile arrival counters followed by the
+ * FP32 partial sums of the shared tiles (padded to whole tiles).  The workspace must be zero-filled
+ * once by the caller before its first use; every call leaves it zero-filled again, so one buffer
+ * serves any sequence of calls on one stream.  Concurrent calls on different streams need their own. */
 size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer);
 
 const char* apex4_status_string(int status);
@@ -110,9 +114,10 @@ int apex4_unpack_codes(const void* q_packed, int R, int K, int operand, int8_t* 
 /* ---- a2..a7: the W4A4 group-dequant GEMM (Eq. 8) ----------------------------- */
 /* Y [M,N] (FP16 or FP32 per out_dtype) = sum_g sA sW P_g.  qA/sA from apex4_quantize_act, qW/sW
  * from apex4_pack_weights, both at the same resolved group size (G_a = G_w).
- * workspace: apex4_workspace_bytes() bytes (may be NULL when that is 0); it is needed when the K loop
- * of an output tile is shared between CTAs (a6: decode-sized M, or a tile count
- * that does not fill the 148 SMs evenly). */
+ * workspace: apex4_workspace_bytes() bytes of DEVICE memory (may be NULL when that is 0); it is used
+ * when the K loop of an output tile is shared between CTAs (a6: a tile count that
+ * does not fill the SMs evenly).  A smaller workspace_bytes returns APEX4_ERR_WORKSPACE and launches
+ * nothing. */
 int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
                     const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
                     int gran, int layer, void* workspace, size_t workspace_bytes, void* stream);
