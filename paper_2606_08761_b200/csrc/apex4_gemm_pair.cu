@@ -12,20 +12,20 @@
 // drains group g; (2) an epilogue thread keeps 96 FP32 running sums, which leaves registers for a
 // true software prefetch of the next TMEM chunk (with 128 sums ptxas serialised load and arithmetic).
 //
-// Roles (640 threads per CTA; launched with 96 registers per thread = the 61 440-register pool that
-// setmaxnreg then redistributes: control 32, wideners 40, epilogue 184):
-//   warps 0-7   wideners : two warpgroups, k-blocks dealt alternately.  INT4 -> INT8 (x16).  Thread r
-//                          widens weight row r in registers and stores it to TMEM; 96 token rows are
-//                          widened smem -> smem into the 128B-swizzled UMMA layout.  One elected
+// Roles (W = 1 or 2 widener warpgroups, template parameter, see Warps<> below; the launch register
+// count x threads is the pool that setmaxnreg redistributes: control 32, wideners 40, epilogue 184-200):
+//   warps 0..4W-1  wideners : k-blocks dealt alternately between the warpgroups.  INT4 -> INT8 (x16).
+//                          Thread r widens weight row r in registers and stores it to TMEM; 96 token
+//                          rows are widened smem -> smem into the 128B-swizzled UMMA layout.  One elected
 //                          arrive per warp on the LEADER's operand barrier.  FP16 -> FP32 scale prep.
-//   warps 8-15  epilogue : warpgroup h owns tokens 96 h .. 96 h + 95.  tcgen05.ld in the 16x256b shape
-//                          (thread = 4 rows x 4 columns of a 16-column chunk, so one LDS.128 fetches
-//                          the four token scales a chunk needs), chunk c+1 in flight while chunk c is
-//                          in the FMA pipe.  Two FFMA2 per element pair: fma(f, sW/256, -49152 sW) =
-//                          P sW rounded once (magic-biased accumulators, see apex4_gemm.cu), then fma
-//                          with sA into the FP32 running sums.
-//   warp 16     producer : 1-D bulk async copies (UBLKCP) of this CTA's packed INT4 rows + FP16 scales
-//   warp 17     MMA      : leader CTA only; tcgen05.mma cta_group::2 kind::i8, M = 256, N = 192, K = 32,
+//   next 8 warps   epilogue : warpgroup h owns tokens 96 h .. 96 h + 95.  tcgen05.ld.32x32b.x16: a thread
+//                          holds one weight row (its TMEM lane) x 16 consecutive tokens per chunk; this
+//                          shape sustains ~1.4 x the TMEM read rate of 16x256b (profiles/r1_ubench_b200.md);
+//                          chunk c+1 is in flight while chunk c is in the FMA pipe.  Two FFMA2 per element
+//                          pair: fma(f, sW/256, -49152 sW) = P sW rounded once (magic-biased accumulators,
+//                          see apex4_gemm.cu), then fma with the two token scales into the FP32 sums.
+//   then           producer : 1-D bulk async copies (UBLKCP) of this CTA's packed INT4 rows + FP16 scales
+//   then           MMA      : leader CTA only; tcgen05.mma cta_group::2 kind::i8, M = 256, N = 192, K = 32,
 //                          A (weights) from TMEM, B (tokens) from shared memory; tcgen05.commit
 //                          multicast to both CTAs.  Producer and MMA loops run warp-uniform with one
 //                          elected lane issuing (operands in uniform registers, no divisions).
@@ -40,13 +40,12 @@ namespace apex4 {
 namespace pair {
 
 constexpr uint32_t kMagicBits = 0x4B400000u;   // float 12582912 = 1.5 * 2^23
-constexpr int kWidenWGs = 2;        // widener warpgroups (k-blocks dealt alternately)
-constexpr int kEpiWarp0 = 4 * kWidenWGs;       // first epilogue warp
-constexpr int kCtlWarp0 = kEpiWarp0 + 8;       // producer warp; the MMA warp follows
-constexpr int kThreads = 32 * (kCtlWarp0 + 4); // warps are allocated in fours: two control warps idle
+constexpr int kEpiWGs = 2;          // epilogue warpgroups (each owns kNT / kEpiWGs token columns)
+constexpr int kEpiWarps = 4 * kEpiWGs;
 constexpr int kNT = kPairTokens;    // 192 tokens per pair tile = MMA N = accumulator buffer width
-constexpr int kHalf = kNT / 2;      // 96 token rows per CTA / columns per epilogue warpgroup
-constexpr int kChunks = kHalf / 16; // 16-column TMEM chunks per epilogue thread
+constexpr int kHalf = kNT / 2;      // 96 token rows per CTA (its half of the B operand)
+constexpr int kEpiCols = kNT / kEpiWGs;        // accumulator columns per epilogue warpgroup
+constexpr int kChunks = kEpiCols / 16;         // 16-column TMEM chunks per epilogue thread
 constexpr int kAccBufs = 2;
 constexpr int kOpStages = 4;        // widened operand stages (TMEM A + smem B)
 constexpr int kPkStages = 6;        // packed (bulk copy) stages
@@ -59,17 +58,44 @@ constexpr int kPkSABytes = 2 * 4 * 256;           // the two 128-token blobs the
 constexpr int kPkStageBytes = kPkWBytes + kPkABytes + kPkSWBytes + kPkSABytes;
 constexpr int kI8StageBytes = kHalf * kBlockK;    // widened tokens: [96 rows][128 B]
 constexpr int kScfSlotBytes = kTileRows * 8 + kNT * 4 + 256;   // {a,b} per row, sA per column (padded)
-constexpr int kRegsCtl = 32, kRegsWiden = 40, kRegsEpi = 184;  // launch: 96 per thread
 constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs;
-constexpr int kStoreBytes = kHalf * 64;            // per epilogue warp: [96 m][32 n] FP16 output staging
+constexpr int kStoreBytes = kEpiCols * 64;         // per epilogue warp: [kEpiCols m][32 n] FP16 output staging
 constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
-                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + 8 * kStoreBytes;
-static_assert((kWidenWGs & (kWidenWGs - 1)) == 0 && (kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
+                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + kEpiWarps * kStoreBytes;
+static_assert((kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
 static_assert((kOpStages & (kOpStages - 1)) == 0, "stage index wraps with a mask");
 static_assert(kAccBufs * kNT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
 static_assert(kI8StageBytes % 1024 == 0 && kPkStageBytes % 16 == 0, "alignment");
 static_assert(kSmemBytes <= 232448, "shared memory");
-static_assert(128 * kRegsCtl + 128 * kWidenWGs * kRegsWiden + 256 * kRegsEpi <= kThreads * 96, "registers");
+static_assert(kNT % (16 * kEpiWGs) == 0, "epilogue warpgroups own whole 16-column chunks");
+
+// Warp layout for WWG widener warpgroups.  With one, the wideners of a CTA run one k-block at a time:
+// fewer warps polling barriers and competing for issue slots, which is what the epilogue-heavy fine
+// granularities want (g <= 128: 903 vs 949 us at 8192^3); with two, k-blocks are dealt alternately and
+// the bulk copy -> widen -> MMA chain is shorter, which is what counts once the epilogue is rare
+// (per-channel, M = 4096, N = K = 8192: 252 vs 294 us).  The register pool is threads x launch
+// registers (<= 64 K), redistributed by setmaxnreg: control 32, wideners 40, the rest to the epilogue.
+template <int WWG>
+struct Warps {
+  static constexpr int kWidenWGs = WWG;                     // k-blocks dealt alternately
+  static constexpr int kEpiWarp0 = 4 * WWG;                 // first epilogue warp
+  static constexpr int kCtlWarp0 = kEpiWarp0 + kEpiWarps;   // producer warp; the MMA warp follows
+  static constexpr int kThreads = 32 * (kCtlWarp0 + 4);     // warps are allocated in fours: two control warps idle
+  static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8 > 120 ? 120 : (65536 / kThreads) / 8 * 8;
+  static constexpr int kRegsCtl = 32, kRegsWiden = 40;
+  static constexpr int kRegsEpi = ((kThreads * kLaunchRegs - 128 * kRegsCtl - 128 * WWG * kRegsWiden) / (128 * kEpiWGs)) / 8 * 8;
+  static_assert((WWG & (WWG - 1)) == 0, "k-blocks are dealt with a mask");
+  static_assert(128 * kRegsCtl + 128 * WWG * kRegsWiden + 128 * kEpiWGs * kRegsEpi <= kThreads * kLaunchRegs, "registers");
+  static_assert(kRegsEpi <= 232 && kThreads <= 1024, "register / thread limits");
+};
+// widener warpgroups for a resolved group size
+inline int widen_wgs(int g) {
+#ifdef APEX4_PAIR_FORCE_WWG   // tuning builds only
+  return APEX4_PAIR_FORCE_WWG;
+#else
+  return g <= kBlockK ? 1 : 2;
+#endif
+}
 
 struct Work {
   int nt, mt;      // pair tile: 256 weight rows, 192 tokens
@@ -112,11 +138,17 @@ __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Wor
 
 using namespace pair;
 
-template <bool BIAS, bool DUMP>
-__global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
+template <bool BIAS, bool DUMP, int WWG>
+__global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
     w4a4_gemm_pair_kernel(const GemmParams p) {
+  using L = Warps<WWG>;
+  constexpr int kWidenWGs = L::kWidenWGs, kEpiWarp0 = L::kEpiWarp0, kCtlWarp0 = L::kCtlWarp0;
+  constexpr int kRegsCtl = L::kRegsCtl, kRegsWiden = L::kRegsWiden, kRegsEpi = L::kRegsEpi;
   extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  // opaque: otherwise ptxas re-derives the base (S2R SR_CgaCtaId + 4 integer ops) in front of every
+  // barrier wait and shared-memory access instead of keeping it in a register
+  uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  asm volatile("" : "+r"(smem_base));
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
 
   constexpr uint32_t offI8 = 0;
@@ -135,7 +167,8 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
   // warp index through a shuffle from lane 0: tells the compiler it is warp-uniform, so addresses derived
   // from it (TMEM lane quarter, barrier and stage addresses) live in uniform registers (no R2UR per use)
   const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
-  const int lane = threadIdx.x & 31;
+  int lane = threadIdx.x & 31;
+  asm volatile("" : "+r"(lane));                // no S2R SR_TID.X inside the loops
   const uint32_t rank = cluster_ctarank();      // 0 = leader
   const int cp = blockIdx.x >> 1;               // pair index
   const int npairs = gridDim.x >> 1;
@@ -155,9 +188,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
     for (int i = 0; i < kPkStages; ++i) { mbar_init(bar(bPkFull + i), 1); mbar_init(bar(bPkEmpty + i), 128); }
     // operand stage full: one elected arrive per widener warp of BOTH CTAs, on the leader's barrier
     for (int i = 0; i < kOpStages; ++i) { mbar_init(bar(bOpFull + i), 8); mbar_init(bar(bOpEmpty + i), 1); }
-    for (int i = 0; i < kScfSlots; ++i) { mbar_init(bar(bScfFull + i), 128); mbar_init(bar(bScfEmpty + i), 8); }
+    for (int i = 0; i < kScfSlots; ++i) { mbar_init(bar(bScfFull + i), 128); mbar_init(bar(bScfEmpty + i), kEpiWarps); }
     // accumulator buffer empty: one elected arrive per epilogue warp of BOTH CTAs, on the leader's barrier
-    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 16); }
+    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 2 * kEpiWarps); }
     fence_mbar_init();
   }
   if (threadIdx.x < 8) reinterpret_cast<volatile uint32_t*>(smem_gen + offMagic)[threadIdx.x] = kMagicBits;
@@ -396,16 +429,13 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
             const float sw = __half2float(sWh[sub * kTileRows + r]);
             // a = sW / 256 (the operands are 16 q each); b = -12582912 * a removes the magic bias
             reinterpret_cast<float2*>(dstf)[r] = make_float2(sw * 0.00390625f, sw * -49152.0f);
-            // token scales, permuted inside every 16-column chunk so that the four columns
-            // {2t, 2t+1, 8+2t, 9+2t} an epilogue thread owns are one 16-byte vector: c -> 4t + 2j + e
+            // token scales, in tile order (an epilogue thread reads the 16 of a chunk as four 16-byte vectors)
 #pragma unroll
             for (int x = 0; x < 2; ++x) {
               const int col = r + 128 * x;                       // token of the tile
               if (col < kNT) {
                 const int mm = sa_off + col;                     // row in the tile's two scale blobs
-                const int c = col & 15;
-                const int pos = (col & ~15) | (((c >> 1) & 3) << 2) | ((c >> 3) << 1) | (c & 1);
-                dstf[2 * kTileRows + pos] = __half2float(sAh[((mm >> 7) * gpk + sub) * kTileRows + (mm & 127)]);
+                dstf[2 * kTileRows + col] = __half2float(sAh[((mm >> 7) * gpk + sub) * kTileRows + (mm & 127)]);
               }
             }
             if (scf_sync) mbar_arrive(bar(bScfFull + q));
@@ -429,18 +459,17 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
   // =========================================================================== epilogue
   else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsEpi));
-    const int h = (warp - kEpiWarp0) >> 2;              // warpgroup = token half
+    const int h = (warp - kEpiWarp0) >> 2;              // warpgroup = slice of kEpiCols token columns
     const int lq = warp & 3;                            // TMEM lane quarter this warp may access
-    const int q = lane >> 2, t = lane & 3;
     const int epi_tid = threadIdx.x - 32 * kEpiWarp0;
     const uint32_t lane_addr = static_cast<uint32_t>(lq * 32) << 16;
-    const int row0 = lq * 32 + q;                       // rows row0 + 8 i, i = 0..3
+    const int row0 = lq * 32 + lane;                    // weight row of the CTA's blob = TMEM lane
     // per-thread address parts of the group loop, made opaque so that ptxas keeps them in registers
     // instead of re-deriving them from %tid in every group (11 S2R + ~40 integer ops per group)
-    uint32_t tm_rd = lane_addr + h * kHalf;                                   // + buf * kNT
-    uint32_t ab_off = offScf + row0 * 8;                                      // {a, b} of row row0 (+ 64 i)
-    uint32_t sa_off = offScf + kTileRows * 8 + (h * kHalf) * 4 + t * 16;      // token scales (+ 64 c)
-    asm volatile("" : "+r"(tm_rd), "+r"(ab_off), "+r"(sa_off));
+    const uint32_t tm_rd = lane_addr + h * kEpiCols;                                   // + buf * kNT
+    uint32_t ab_off = offScf + row0 * 8;                                      // {a, b} of row row0
+    uint32_t sa_off = offScf + kTileRows * 8 + (h * kEpiCols) * 4;            // token scales (+ 64 c)
+    asm volatile("" : "+r"(ab_off), "+r"(sa_off));   // tm_rd stays warp-uniform (uniform registers)
     // the magic bias in 8 registers, read through a volatile load so that ptxas keeps them resident
     // instead of re-materialising 16 constants per tcgen05.st (IMAD.MOV on the FMA pipe)
     uint32_t mg[8];
@@ -454,7 +483,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
     for (int b = 0; b < kAccBufs; ++b) {
       if (BIAS) {
 #pragma unroll
-        for (int c = 0; c < kHalf; c += 8) tmem_st_32x8(tmem_base + lane_addr + b * kNT + h * kHalf + c, mg);
+        for (int c = 0; c < kEpiCols; c += 8) tmem_st_32x8(tmem_base + lane_addr + b * kNT + h * kEpiCols + c, mg);
         tmem_st_wait();
       }
       tc_fence_before();
@@ -467,11 +496,11 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       if (epi_tid == 0) stamp(15, item * 4);
       const int nkb = w.kb1 - w.kb0;
       const int ngroups = g < kBlockK ? nkb * gpk : nkb / kbpg;
-      uint64_t acc[8 * kChunks];                        // [i][c][j] -> (i * kChunks + c) * 2 + j
+      uint64_t acc[8 * kChunks];                        // FP32 pairs: tokens 2 x, 2 x + 1 of the slice
 #pragma unroll
       for (int i = 0; i < 8 * kChunks; ++i) acc[i] = 0ull;
       const int n_glob0 = (2 * w.nt + static_cast<int>(rank)) * kTileRows + row0;
-      const int m_glob0 = w.mt * kNT + h * kHalf + 2 * t;   // + 16 c + 8 j + e
+      const int m_glob0 = w.mt * kNT + h * kEpiCols;        // + 16 c + j
 
       for (int gi = 0; gi < ngroups; ++gi, ++gc) {
         const int slot = gc % kScfSlots;
@@ -479,73 +508,61 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
         if (scf_sync) mbar_wait(bar(bScfFull + slot), (gc / kScfSlots) & 1);
         mbar_wait(bar(bAccFull + buf), (gc >> 1) & 1);
         const uint32_t scf = smem_base + slot * kScfSlotBytes;
-        uint64_t a2[4], b2[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        {
+          // ---- this thread = weight row row0 (TMEM lane), 16 consecutive tokens per chunk
           float af, bf;
-          unpack_f2(lds64(scf + ab_off + 64 * i), af, bf);
-          a2[i] = pack_f2(af, af);
-          b2[i] = pack_f2(bf, bf);
-        }
-        const uint32_t sAf = scf + sa_off;   // + 64 c
-        tc_fence_after();
-        if (epi_tid == 0) stamp(6, gc);
-        const uint32_t tb = tm_rd + buf * kNT;
-        uint32_t v[2][16];
-        uint64_t sq[2][2];                               // token scales of chunk c, c + 1
-        lds_2x64(sAf, sq[0][0], sq[0][1]);
-        tmem_ld_16x256b_x2(tb, v[0]);
-        tmem_ld_16x256b_x2(tb + (16u << 16), v[0] + 8);
+          unpack_f2(lds64(scf + ab_off), af, bf);
+          const uint64_t a2 = pack_f2(af, af), b2 = pack_f2(bf, bf);
+          const uint32_t sAf = scf + sa_off;   // + 64 c
+          tc_fence_after();
+          if (epi_tid == 0) stamp(6, gc);
+          const uint32_t tb = tm_rd + buf * kNT;
+          uint32_t v[2][16];
+          uint64_t sq[8];                                  // token scales of the chunk, as pairs
+          tmem_ld_32x16(tb, v[0]);
 #pragma unroll
-        for (int c = 0; c < kChunks; ++c) {
-          uint32_t* vc = v[c & 1];
-          tmem_ld_wait16(vc);
-          if (c < kChunks - 1) {                         // prefetch chunk c + 1, then re-arm chunk c
-            tmem_ld_16x256b_x2(tb + 16 * (c + 1), v[(c + 1) & 1]);
-            tmem_ld_16x256b_x2(tb + (16u << 16) + 16 * (c + 1), v[(c + 1) & 1] + 8);
-            lds_2x64(sAf + 64 * (c + 1), sq[(c + 1) & 1][0], sq[(c + 1) & 1][1]);
-          }
-          if constexpr (BIAS) {
-            tmem_st_32x8(tb + 16 * c, mg);
-            tmem_st_32x8(tb + 16 * c + 8, mg);
-          }
-          if (c == kChunks - 1) {                        // buffer fully read (and re-armed): hand it back
-            if constexpr (BIAS) tmem_st_wait();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + buf), 0);
-          }
-          if constexpr (DUMP) {
-            const int gamma = (g < kBlockK ? w.kb0 * gpk : w.kb0 / kbpg) + gi;
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-              for (int j = 0; j < 2; ++j)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  const int m = m_glob0 + 16 * c + 8 * j + e;
-                  const int n = n_glob0 + 8 * i;
-                  if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1) {
-                    const uint32_t x = vc[8 * (i >> 1) + 4 * j + 2 * (i & 1) + e];
-                    const int32_t raw = static_cast<int32_t>(BIAS ? x - kMagicBits : x);
-                    p.P_out[(static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gamma] = raw >> 8;
-                  }
-                }
-          }
-          const uint64_t s01 = sq[c & 1][0], s23 = sq[c & 1][1];   // columns {2t,2t+1}, {8+2t,9+2t}
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int rb = 8 * (i >> 1) + 2 * (i & 1);
-            uint64_t t0, t1;
+          for (int c = 0; c < kChunks; ++c) {
+            uint32_t* vc = v[c & 1];
+            // the scales of chunk c (those of chunk c - 1 have been consumed): in flight during the wait
+            lds_2x64(sAf + 64 * c, sq[0], sq[1]);
+            lds_2x64(sAf + 64 * c + 16, sq[2], sq[3]);
+            lds_2x64(sAf + 64 * c + 32, sq[4], sq[5]);
+            lds_2x64(sAf + 64 * c + 48, sq[6], sq[7]);
+            tmem_ld_wait16(vc);
+            if (c < kChunks - 1) tmem_ld_32x16(tb + 16 * (c + 1), v[(c + 1) & 1]);
             if constexpr (BIAS) {
-              t0 = fma2v(pack_u2(vc[rb], vc[rb + 1]), a2[i], b2[i]);
-              t1 = fma2v(pack_u2(vc[rb + 4], vc[rb + 5]), a2[i], b2[i]);
-            } else {
-              t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[rb])), __int2float_rn(static_cast<int>(vc[rb + 1]))), a2[i]);
-              t1 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[rb + 4])), __int2float_rn(static_cast<int>(vc[rb + 5]))), a2[i]);
+              tmem_st_32x8(tb + 16 * c, mg);
+              tmem_st_32x8(tb + 16 * c + 8, mg);
             }
-            acc[(i * kChunks + c) * 2] = fma2(t0, s01, acc[(i * kChunks + c) * 2]);
-            acc[(i * kChunks + c) * 2 + 1] = fma2(t1, s23, acc[(i * kChunks + c) * 2 + 1]);
+            if (c == kChunks - 1) {                        // buffer fully read (and re-armed): hand it back
+              if constexpr (BIAS) tmem_st_wait();
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + buf), 0);
+            }
+            if constexpr (DUMP) {
+              const int gamma = (g < kBlockK ? w.kb0 * gpk : w.kb0 / kbpg) + gi;
+#pragma unroll
+              for (int j = 0; j < 16; ++j) {
+                const int m = m_glob0 + 16 * c + j;
+                const int n = n_glob0;
+                if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1) {
+                  const uint32_t x = vc[j];
+                  const int32_t raw = static_cast<int32_t>(BIAS ? x - kMagicBits : x);
+                  p.P_out[(static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gamma] = raw >> 8;
+                }
+              }
+            }
+#pragma unroll
+            for (int jj = 0; jj < 8; ++jj) {
+              uint64_t t0;
+              if constexpr (BIAS) {
+                t0 = fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2);
+              } else {
+                t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[2 * jj])), __int2float_rn(static_cast<int>(vc[2 * jj + 1]))), a2);
+              }
+              acc[c * 8 + jj] = fma2(t0, sq[jj], acc[c * 8 + jj]);   // tokens 16 c + 2 jj, + 1
+            }
           }
         }
         if (scf_sync) {
@@ -560,54 +577,44 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
       if (p.Y != nullptr) {
         auto store_tile = [&]() {
           if (!p.out_f32) {
-            // FP16 output: the warp's 32 (n) x 96 (m) sub-tile is transposed through a private 6 KB
-            // shared-memory tile [m][32 n] (16-byte part p of row m stored at p ^ ((m >> 1) & 3): both the
-            // 2-byte scatter and the 16-byte gather are bank-conflict free), then written as 16-byte
+            // FP16 output: the warp's 32 (n) x 96 (m) sub-tile goes through a private 6 KB shared-memory
+            // tile [m][32 n] (16-byte part p of row m stored at p ^ ((m >> 1) & 3)), then out as 16-byte
             // row pieces: 12 STG.128 per thread instead of 96 STG.U16 with 64-bit address arithmetic
             // (the store phase was 10-12 % of the config-1 GEMM time)
             const uint32_t stg = smem_base + offStore + (warp - kEpiWarp0) * kStoreBytes;
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-              for (int c = 0; c < kChunks; ++c)
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                  float f0, f1;
-                  unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
-                  const uint32_t a0 = stg + (16 * c + 8 * j + 2 * t) * 64 + ((i ^ t) << 4) + 2 * q;   // row m, column n = q + 8 i
-                  asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0), "h"(__half_as_ushort(__float2half_rn(f0))) : "memory");
-                  asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0 + 64), "h"(__half_as_ushort(__float2half_rn(f1))) : "memory");
-                }
+            for (int x = 0; x < 8 * kChunks; ++x) {       // tokens m = 2 x, 2 x + 1 of the warpgroup's slice, n = lane
+              float f0, f1;
+              unpack_f2(acc[x], f0, f1);
+              const uint32_t a0 = stg + (2 * x) * 64 + (((lane >> 3) ^ (x & 3)) << 4) + 2 * (lane & 7);
+              asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0), "h"(__half_as_ushort(__float2half_rn(f0))) : "memory");
+              asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0 + 64), "h"(__half_as_ushort(__float2half_rn(f1))) : "memory");
+            }
             __syncwarp();
             const int n = (2 * w.nt + static_cast<int>(rank)) * kTileRows + lq * 32 + (lane & 3) * 8;
             __half* ybase = static_cast<__half*>(p.Y) + n;
 #pragma unroll
-            for (int ps = 0; ps < kHalf / 8; ++ps) {
+            for (int ps = 0; ps < kEpiCols / 8; ++ps) {
               const int row = ps * 8 + (lane >> 2);
               uint32_t x0, x1, x2, x3;
               lds128(stg + row * 64 + (((lane & 3) ^ ((row >> 1) & 3)) << 4), x0, x1, x2, x3);
-              const int m = w.mt * kNT + h * kHalf + row;
+              const int m = w.mt * kNT + h * kEpiCols + row;
               if (m < p.M && n < p.N)
                 *reinterpret_cast<uint4*>(ybase + static_cast<size_t>(m) * p.N) = make_uint4(x0, x1, x2, x3);
             }
             __syncwarp();
             return;
           }
+          float* y = static_cast<float*>(p.Y);      // FP32 output: lanes = consecutive n, coalesced rows
+          if (n_glob0 < p.N) {
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int n = n_glob0 + 8 * i;
-            if (n >= p.N) continue;
-#pragma unroll
-            for (int c = 0; c < kChunks; ++c)
-#pragma unroll
-              for (int j = 0; j < 2; ++j) {
-                float f0, f1;
-                unpack_f2(acc[(i * kChunks + c) * 2 + j], f0, f1);
-                const int m = m_glob0 + 16 * c + 8 * j;
-                float* y = static_cast<float*>(p.Y);
-                if (m < p.M) y[static_cast<size_t>(m) * p.N + n] = f0;
-                if (m + 1 < p.M) y[static_cast<size_t>(m + 1) * p.N + n] = f1;
-              }
+            for (int x = 0; x < 8 * kChunks; ++x) {
+              float f0, f1;
+              unpack_f2(acc[x], f0, f1);
+              const int m = m_glob0 + 2 * x;
+              if (m < p.M) y[static_cast<size_t>(m) * p.N + n_glob0] = f0;
+              if (m + 1 < p.M) y[static_cast<size_t>(m + 1) * p.N + n_glob0] = f1;
+            }
           }
         };
         if (!w.partial) {
@@ -625,14 +632,14 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
             float f0, f1, f2, f3;
             unpack_f2(acc[2 * j], f0, f1);
             unpack_f2(acc[2 * j + 1], f2, f3);
-            asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(wst + j * 1024), "f"(f0),
+            asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(wst + j * (128 * kEpiWarps)), "f"(f0),
                          "f"(f1), "f"(f2), "f"(f3)
                          : "memory");
           }
           __threadfence();
           if (epi_tid == 0) stamp(15, item * 4 + 2);
           int* flag = reinterpret_cast<int*>(smem_gen + offTmemPtr + 8);
-          asm volatile("bar.sync 1, 256;" ::: "memory");
+          asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
           if (epi_tid == 0) {
             const int tile = (w.nt * p.tiles_m + w.mt) * 2 + static_cast<int>(rank);
             const int prev = atomicAdd(p.counters + tile, w.units);
@@ -640,19 +647,19 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
             *flag = done;
             if (done) p.counters[tile] = 0;
           }
-          asm volatile("bar.sync 1, 256;" ::: "memory");
+          asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
           const int done = *flag;
-          asm volatile("bar.sync 1, 256;" ::: "memory");   // flag may be rewritten by the next item
+          asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");   // flag may be rewritten by the next item
           if (done) {
             __threadfence();
 #pragma unroll
             for (int j = 0; j < 4 * kChunks; ++j) {       // all loads first, then the zero stores
-              const float4 x = __ldcg(reinterpret_cast<const float4*>(wst + j * 1024));
+              const float4 x = __ldcg(reinterpret_cast<const float4*>(wst + j * (128 * kEpiWarps)));
               acc[2 * j] = pack_f2(x.x, x.y);
               acc[2 * j + 1] = pack_f2(x.z, x.w);
             }
 #pragma unroll
-            for (int j = 0; j < 4 * kChunks; ++j) __stcg(reinterpret_cast<float4*>(wst + j * 1024), make_float4(0.f, 0.f, 0.f, 0.f));
+            for (int j = 0; j < 4 * kChunks; ++j) __stcg(reinterpret_cast<float4*>(wst + j * (128 * kEpiWarps)), make_float4(0.f, 0.f, 0.f, 0.f));
             store_tile();
           }
         }
@@ -673,29 +680,33 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(96)
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <bool BIAS, bool DUMP>
+template <bool BIAS, bool DUMP, int WWG>
 static cudaError_t launch_pair_one(const GemmParams& p, int npairs, cudaStream_t st) {
-  auto kern = w4a4_gemm_pair_kernel<BIAS, DUMP>;
+  auto kern = w4a4_gemm_pair_kernel<BIAS, DUMP, WWG>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
   if (e != cudaSuccess) return e;
-  kern<<<2 * npairs, kThreads, kSmemBytes, st>>>(p);
+  kern<<<2 * npairs, Warps<WWG>::kThreads, kSmemBytes, st>>>(p);
   return cudaGetLastError();
+}
+template <int WWG>
+static cudaError_t launch_pair_w(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
+  if (bias) return dump ? launch_pair_one<true, true, WWG>(p, npairs, st) : launch_pair_one<true, false, WWG>(p, npairs, st);
+  return dump ? launch_pair_one<false, true, WWG>(p, npairs, st) : launch_pair_one<false, false, WWG>(p, npairs, st);
 }
 
 cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
-  if (bias) return dump ? launch_pair_one<true, true>(p, npairs, st) : launch_pair_one<true, false>(p, npairs, st);
-  return dump ? launch_pair_one<false, true>(p, npairs, st) : launch_pair_one<false, false>(p, npairs, st);
+  return widen_wgs(p.g) == 1 ? launch_pair_w<1>(p, bias, dump, npairs, st) : launch_pair_w<2>(p, bias, dump, npairs, st);
 }
 
 // CTA pairs that can be resident at once (one per TPC); queried once
 int gemm_max_pairs() {
   static int pairs = 0;
   if (pairs == 0) {
-    auto kern = w4a4_gemm_pair_kernel<true, false>;
+    auto kern = w4a4_gemm_pair_kernel<true, false, 2>;   // one CTA per SM whatever the warp layout
     int n = 0;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(2 * 74);
-    cfg.blockDim = dim3(kThreads);
+    cfg.blockDim = dim3(Warps<2>::kThreads);
     cfg.dynamicSmemBytes = kSmemBytes;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
