@@ -55,6 +55,46 @@ __device__ __forceinline__ uint4 quant_pack_chunk(const uint4 (&v)[4], float s, 
   return make_uint4(out[0], out[1], out[2], out[3]);
 }
 
+// The same 16 bytes without a division per element.  rne(x / s) is decided from two products that
+// bracket the true quotient, x * inv * (1 -/+ 2^-20) with inv = rn(1 / s): each FFMA adds 1.5 * 2^23, so
+// the FP32 rounding of the sum IS round-half-to-even to an integer, and its low mantissa nibble is the
+// two's-complement code.  Rounding is monotonic, so when both ends give the same integer the true
+// quotient (and by lemma L1 the binary32 quotient of quant_one) rounds to it too.  When they differ for
+// any element of the chunk (the quotient is within ~1e-5 of a half-integer: ~5e-4 of all chunks), or S
+// is an FP16 subnormal (only then can |x / S| exceed 7.5 and the clamp of Eq. 7 act), the chunk is
+// redone by quant_pack_chunk with IEEE divisions.  Codes are bit-identical to quant_pack_chunk's.
+__device__ __forceinline__ uint4 quant_pack_chunk_fast(const uint4 (&v)[4], float s, int swap) {
+  if (s == 0.f) return make_uint4(0u, 0u, 0u, 0u);
+  if (s < 6.103515625e-05f) return quant_pack_chunk(v, s, swap);   // S below 2^-14
+  const float inv = __frcp_rn(s);
+  const float inv_lo = inv * 0.99999904632568359375f;   // 1 - 2^-20
+  const float inv_hi = inv * 1.00000095367431640625f;   // 1 + 2^-20
+  const float magic = 12582912.0f;                      // 1.5 * 2^23: ulp 1, integer in the mantissa
+  const uint32_t* w = reinterpret_cast<const uint32_t*>(v);
+  uint32_t chk = 0;
+  uint32_t byte[16];                                    // byte y = element y (low nibble), 16 + y (high)
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const float2 fa = __half22float2(*reinterpret_cast<const __half2*>(&w[swap ? 8 + i : i]));
+    const float2 fb = __half22float2(*reinterpret_cast<const __half2*>(&w[swap ? i : 8 + i]));
+    const uint32_t a0 = __float_as_uint(__fmaf_rn(fa.x, inv_lo, magic)), a0h = __float_as_uint(__fmaf_rn(fa.x, inv_hi, magic));
+    const uint32_t a1 = __float_as_uint(__fmaf_rn(fa.y, inv_lo, magic)), a1h = __float_as_uint(__fmaf_rn(fa.y, inv_hi, magic));
+    const uint32_t b0 = __float_as_uint(__fmaf_rn(fb.x, inv_lo, magic)), b0h = __float_as_uint(__fmaf_rn(fb.x, inv_hi, magic));
+    const uint32_t b1 = __float_as_uint(__fmaf_rn(fb.y, inv_lo, magic)), b1h = __float_as_uint(__fmaf_rn(fb.y, inv_hi, magic));
+    chk |= (a0 ^ a0h) | (a1 ^ a1h);
+    chk |= (b0 ^ b0h) | (b1 ^ b1h);
+    byte[2 * i] = (a0 & 0xFu) | (b0 << 4);              // bits 8.. are junk, dropped by the byte gather
+    byte[2 * i + 1] = (a1 & 0xFu) | (b1 << 4);
+  }
+  if (chk != 0) return quant_pack_chunk(v, s, swap);
+  uint32_t out[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    out[i] = __byte_perm(__byte_perm(byte[4 * i], byte[4 * i + 1], 0x0040),
+                         __byte_perm(byte[4 * i + 2], byte[4 * i + 3], 0x0040), 0x5410);
+  return make_uint4(out[0], out[1], out[2], out[3]);
+}
+
 __device__ __forceinline__ float scale_from_absmax_bits(uint32_t amax_bits, __half* S_out) {
   __half a = __ushort_as_half(static_cast<unsigned short>(amax_bits));
   float s32 = __fdiv_rn(__half2float(a), 7.0f);
@@ -104,7 +144,7 @@ __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __r
   }
   __half Sh;
   const float s = scale_from_absmax_bits(m, &Sh);
-  const uint4 packed = quant_pack_chunk(v, s, weights ? 0 : (r & 1));
+  const uint4 packed = quant_pack_chunk_fast(v, s, weights ? 0 : (r & 1));
   if (active) {
     *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c, K)) = packed;
     if ((c % GL) == 0) S[st16_index(r, c / GL, cpr / GL)] = Sh;
@@ -163,7 +203,7 @@ __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
   for (int u = 0; u < kLargeUnroll; ++u) {
     const int cl = threadIdx.x + u * kLargeThreads;
     if (cl < cpg) {
-      const uint4 packed = quant_pack_chunk(v[u], s, weights ? 0 : (r & 1));
+      const uint4 packed = quant_pack_chunk_fast(v[u], s, weights ? 0 : (r & 1));
       *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c0 + cl, K)) = packed;
     }
   }
