@@ -115,13 +115,15 @@ template <int GL>
 __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __restrict__ X, int R,
                                                                int K, uint8_t* __restrict__ q,
                                                                __half* __restrict__ S, int weights) {
-  const int cpr = K / 32;
-  const long long total = static_cast<long long>(R) * cpr;
-  long long gid = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  // 32-bit chunk index (the launcher checks R * K / 32 < 2^32): a 64-bit division here was ~150 of the
+  // ~500 instructions of a thread
+  const uint32_t cpr = static_cast<uint32_t>(K) / 32u;
+  const uint32_t total = static_cast<uint32_t>(R) * cpr;
+  uint32_t gid = blockIdx.x * 256u + threadIdx.x;
   const bool active = gid < total;
   if (!active) gid = total - 1;   // keep the warp converged for the shuffles; results discarded
   const int r = static_cast<int>(gid / cpr);
-  const int c = static_cast<int>(gid % cpr);
+  const int c = static_cast<int>(gid - static_cast<uint32_t>(r) * cpr);
   const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + c * 32);
   uint4 v[4];
 #pragma unroll
@@ -291,6 +293,7 @@ cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s
   const unsigned blocks = static_cast<unsigned>((total + 255) / 256);
   const bool pow2 = (gl & (gl - 1)) == 0;
   if (pow2 && gl <= 32) {
+    if (total + 256 > 0xFFFFFFFFll) return cudaErrorInvalidValue;   // 32-bit chunk index in the kernel
     switch (gl) {
       case 1: quantize_small_g_kernel<1><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
       case 2: quantize_small_g_kernel<2><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;

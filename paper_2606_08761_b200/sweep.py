@@ -1,5 +1,6 @@
 """Shape sweeps behind `bench.py --sweep`: BASELINE.json config 2 (N = K = 8192, g = 128,
-M from decode to prefill), config 3 (granularities at M = 4096) and config 4 (Llama-2-70B linears at
+M from decode to prefill), config 3 (granularities at M = 4096, incl. g = 256 / 512 / 1024 and the Fig. 11 g128 / per-channel
+ratio over M) and config 4 (Llama-2-70B linears at
 M = 1, 16, 256, 4096).  Per shape: GEMM time, effective TOPS (2MNK/t), the fraction of
 the roofline that binds (INT8 tensor peak for M >= 256, HBM copy bandwidth below), and the speed-up
 over cuBLAS FP16 (`torch.matmul`) on the same (M, N, K).
@@ -92,7 +93,9 @@ def run_sweeps(dev, peaks=None):
     # slower (M = 16, N = K = 8192: 16.2 vs 11.2 us; M = 256, N = 8192, K = 28672: 335 vs 180 us).
     shapes70 = ((10240, 8192), (8192, 8192), (57344, 8192), (8192, 28672))
     jobs = [("cfg2", M, 8192, 8192, 128, True) for M in (1, 4, 16, 64, 256, 1024, 4096, 8192)]
-    jobs += [("cfg3", 4096, 8192, 8192, g, False) for g in (32, 64, 128, 8192)]
+    jobs += [("cfg3", 4096, 8192, 8192, g, False) for g in (32, 64, 128, 256, 512, 1024, 8192)]
+    # Fig. 11: g = 128 against per-channel over M at N = K = 8192
+    jobs += [("fig11", M, 8192, 8192, g, False) for M in (1024, 2048, 4096, 8192, 16384, 32768) for g in (128, 8192)]
     jobs += [("cfg4", M, N, K, 128, True) for M in (1, 16, 256, 4096) for (N, K) in shapes70]
     done = {}
     for i in sorted(range(len(jobs)), key=lambda i: jobs[i][1] * jobs[i][2] * jobs[i][3]):
@@ -119,4 +122,10 @@ def run_sweeps(dev, peaks=None):
         "baseline_mix_fine128_us": round((2 * t[128] + 5 * t[8192]) / 7, 2),
         "uniform_g128_us": t[128]}
     res["config4_llama70b"] = cfg4
+    f11 = {(jobs[i][1], jobs[i][4]): done[i] for i in range(len(jobs)) if jobs[i][0] == "fig11"}
+    res["fig11_g128_over_channel"] = [
+        {"M": M, "g128_us": f11[(M, 128)]["us"], "channel_us": f11[(M, 8192)]["us"],
+         "g128_tops": f11[(M, 128)]["tops"], "channel_tops": f11[(M, 8192)]["tops"],
+         "ratio": round(f11[(M, 128)]["us"] / f11[(M, 8192)]["us"], 3)}
+        for M in sorted({k[0] for k in f11})]
     return res
