@@ -157,6 +157,7 @@ __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __r
 // the absmax pass and the quantize pass.
 constexpr int kLargeThreads = 256;
 constexpr int kLargeUnroll = 4;
+template <int U>   // chunks per thread (1, 2 or kLargeUnroll): fewer live registers, more blocks per SM
 __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
     const __half* __restrict__ X, int R, int K, int g, uint8_t* __restrict__ q,
     __half* __restrict__ S, int weights) {
@@ -166,11 +167,12 @@ __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
   const int cpg = g / 32;
   const int c0 = gamma * cpg;
   __shared__ uint32_t red[kLargeThreads / 32];
-  uint4 v[kLargeUnroll][4];
+  const int nthr = blockDim.x;          // min(256, chunks per group rounded up to a warp): no idle warps
+  uint4 v[U][4];
   uint32_t m = 0;
 #pragma unroll
-  for (int u = 0; u < kLargeUnroll; ++u) {
-    const int cl = threadIdx.x + u * kLargeThreads;
+  for (int u = 0; u < U; ++u) {
+    const int cl = threadIdx.x + u * nthr;
     if (cl < cpg) {
       const uint4* src =
           reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + (c0 + cl) * 32);
@@ -194,16 +196,15 @@ __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
   if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
   __syncthreads();
   m = red[0];
-#pragma unroll
-  for (int i = 1; i < kLargeThreads / 32; ++i)
+  for (int i = 1; i < nthr / 32; ++i)
     m = __half_as_ushort(__hmax(__ushort_as_half(static_cast<unsigned short>(m)),
                                 __ushort_as_half(static_cast<unsigned short>(red[i]))));
   __half Sh;
   const float s = scale_from_absmax_bits(m, &Sh);
   if (threadIdx.x == 0) S[st16_index(r, gamma, G)] = Sh;
 #pragma unroll
-  for (int u = 0; u < kLargeUnroll; ++u) {
-    const int cl = threadIdx.x + u * kLargeThreads;
+  for (int u = 0; u < U; ++u) {
+    const int cl = threadIdx.x + u * nthr;
     if (cl < cpg) {
       const uint4 packed = quant_pack_chunk_fast(v[u], s, weights ? 0 : (r & 1));
       *reinterpret_cast<uint4*>(q + chunk_dst_offset(r, c0 + cl, K)) = packed;
@@ -305,7 +306,11 @@ cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s
   } else {
     if (gl > kLargeThreads * kLargeUnroll) return cudaErrorInvalidValue;
     const long long nb = static_cast<long long>(R) * (K / g);
-    quantize_large_g_kernel<<<static_cast<unsigned>(nb), kLargeThreads, 0, st>>>(X, R, K, g, Q, S, weights);
+    const int threads = gl >= kLargeThreads ? kLargeThreads : (gl + 31) / 32 * 32;
+    const unsigned nbu = static_cast<unsigned>(nb);
+    if (gl <= kLargeThreads) quantize_large_g_kernel<1><<<nbu, threads, 0, st>>>(X, R, K, g, Q, S, weights);
+    else if (gl <= 2 * kLargeThreads) quantize_large_g_kernel<2><<<nbu, threads, 0, st>>>(X, R, K, g, Q, S, weights);
+    else quantize_large_g_kernel<kLargeUnroll><<<nbu, threads, 0, st>>>(X, R, K, g, Q, S, weights);
   }
   return cudaGetLastError();
 }

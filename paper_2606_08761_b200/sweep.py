@@ -1,7 +1,8 @@
 """Shape sweeps behind `bench.py --sweep`: BASELINE.json config 2 (N = K = 8192, g = 128,
 M from decode to prefill), config 3 (granularities at M = 4096, incl. g = 256 / 512 / 1024 and the Fig. 11 g128 / per-channel
-ratio over M) and config 4 (Llama-2-70B linears at
-M = 1, 16, 256, 4096).  Per shape: GEMM time, effective TOPS (2MNK/t), the fraction of
+ratio over M), config 4 (Llama-2-70B linears at
+M = 1, 16, 256, 4096) and whole-block times of Llama-2-7B / Qwen2.5-7B under the granularity
+policies.  Per shape: GEMM time, effective TOPS (2MNK/t), the fraction of
 the roofline that binds (INT8 tensor peak for M >= 256, HBM copy bandwidth below), and the speed-up
 over cuBLAS FP16 (`torch.matmul`) on the same (M, N, K).
 
@@ -85,6 +86,77 @@ def time_shape(M, N, K, g, dev, cublas=True):
     return out
 
 
+def time_quant(M, K, g, dev):
+    """Activation quantizer (a1) alone, same protocol; rotating inputs larger than L2."""
+    nsets = int(max(2, min(8, 2 * L2_BYTES // (2 * M * K) + 1)))
+    xs = [torch.randn(M, K, device=dev, dtype=torch.float16) for _ in range(nsets)]
+    q = torch.empty(apex4.packed_bytes(M, K), dtype=torch.uint8, device=dev)
+    s = torch.empty(apex4.scale_elems(M, K, g), dtype=torch.float16, device=dev)
+    us = _graph_time_us(lambda i: apex4.quantize_act(xs[i], g, q=q, s=s), nsets)
+    del xs
+    torch.cuda.empty_cache()
+    return us
+
+
+# One transformer block's linears, (hidden, kv width, intermediate); shapes from the public model configs,
+# weights not needed (SURVEY 8(f) item 3; PAPER.md:343 evaluates both models end to end).
+BLOCK_MODELS = {"llama-2-7b": (4096, 4096, 11008), "qwen2.5-7b": (3584, 512, 18944)}
+
+
+def block_ops(h, kv, inter, policy):
+    """-> (quantizer calls [(K, gran, layer)], GEMMs [(name, N, K, gran, layer)]) of one block under a policy.
+    G_a = G_w: an activation is quantized once per distinct granularity its consumers
+    use, so the paper's mix (V and DOWN fine, the rest per-channel, R11) splits V off the fused QKV GEMM
+    and quantizes the block input twice."""
+    A = apex4
+    if policy == "uniform_g128":
+        gr = A.GRAN_GROUP
+        return ([(h, gr, A.LAYER_QKV), (h, gr, A.LAYER_O), (h, gr, A.LAYER_GATE_UP), (inter, gr, A.LAYER_DOWN)],
+                [("qkv", h + 2 * kv, h, gr, A.LAYER_QKV), ("o", h, h, gr, A.LAYER_O),
+                 ("gate_up", 2 * inter, h, gr, A.LAYER_GATE_UP), ("down", h, inter, gr, A.LAYER_DOWN)])
+    if policy == "uniform_channel":
+        gr = A.GRAN_CHANNEL
+        return ([(h, gr, A.LAYER_QKV), (h, gr, A.LAYER_O), (h, gr, A.LAYER_GATE_UP), (inter, gr, A.LAYER_DOWN)],
+                [("qkv", h + 2 * kv, h, gr, A.LAYER_QKV), ("o", h, h, gr, A.LAYER_O),
+                 ("gate_up", 2 * inter, h, gr, A.LAYER_GATE_UP), ("down", h, inter, gr, A.LAYER_DOWN)])
+    gr = A.GRAN_MIXED if policy == "mixed_fine32" else A.GRAN_MIXED_G128
+    return ([(h, gr, A.LAYER_Q), (h, gr, A.LAYER_V), (h, gr, A.LAYER_O), (h, gr, A.LAYER_GATE_UP),
+             (inter, gr, A.LAYER_DOWN)],
+            [("qk", h + kv, h, gr, A.LAYER_Q), ("v", kv, h, gr, A.LAYER_V), ("o", h, h, gr, A.LAYER_O),
+             ("gate_up", 2 * inter, h, gr, A.LAYER_GATE_UP), ("down", h, inter, gr, A.LAYER_DOWN)])
+
+
+def run_block_policies(dev, M=2048):
+    """Whole-block time (every quantizer call + every GEMM of one transformer block, each timed with the
+    sweep protocol and summed) per model and granularity policy; g comes from apex4_resolve_group_size."""
+    res = []
+    cache = {}
+    for model, (h, kv, inter) in BLOCK_MODELS.items():
+        for policy in ("uniform_g128", "mixed_fine32", "mixed_fine128", "uniform_channel"):
+            quants, gemms = block_ops(h, kv, inter, policy)
+            ops, total, work = [], 0.0, 0.0
+            for (K, gran, layer) in quants:
+                g = apex4.resolve_group_size(K, 128, gran, layer)
+                key = ("q", M, K, g)
+                if key not in cache:
+                    time.sleep(0.2)
+                    cache[key] = time_quant(M, K, g, dev)
+                ops.append({"op": "quantize", "K": K, "g": g, "us": round(cache[key], 2)})
+                total += cache[key]
+            for (name, N, K, gran, layer) in gemms:
+                g = apex4.resolve_group_size(K, 128, gran, layer)
+                key = ("g", M, N, K, g)
+                if key not in cache:
+                    time.sleep(0.2)
+                    cache[key] = time_shape(M, N, K, g, dev, cublas=False)["us"]
+                ops.append({"op": name, "N": N, "K": K, "g": g, "us": cache[key]})
+                total += cache[key]
+                work += 2.0 * M * N * K
+            res.append({"model": model, "policy": policy, "M": M, "block_us": round(total, 1),
+                        "tops": round(work / total * 1e-6, 1), "ops": ops})
+    return res
+
+
 def run_sweeps(dev, peaks=None):
     """-> dict of lists; `peaks` = {"hbm": GB/s, "int8": TOP/s} adds the roofline fractions."""
     res = {"protocol": f"CUDA graph of {GRAPH_LAUNCHES} launches rotating operand sets larger than L2, median of 10 replays"}
@@ -122,6 +194,7 @@ def run_sweeps(dev, peaks=None):
         "baseline_mix_fine128_us": round((2 * t[128] + 5 * t[8192]) / 7, 2),
         "uniform_g128_us": t[128]}
     res["config4_llama70b"] = cfg4
+    res["block_policies"] = run_block_policies(dev)
     f11 = {(jobs[i][1], jobs[i][4]): done[i] for i in range(len(jobs)) if jobs[i][0] == "fig11"}
     res["fig11_g128_over_channel"] = [
         {"M": M, "g128_us": f11[(M, 128)]["us"], "channel_us": f11[(M, 8192)]["us"],

@@ -238,6 +238,36 @@ def test_gemm_sampled_large(A):
         assert np.array_equal(P, O.group_sums(qa[m0:m0 + 8], qw[n0:n0 + 8], g))
 
 
+@pytest.mark.parametrize("N,K,layer,g_expect", [
+    (512, 3584, "LAYER_V", 32),          # Qwen2.5-7B V-proj (4 KV heads x 128), paper mix: fine
+    (4096, 3584, "LAYER_Q", 3584),       # fused Q+K, paper mix: per-channel
+    (3584, 18944, "LAYER_DOWN", 32),     # down-proj, paper mix: fine, K = 148 k-blocks
+])
+def test_gemm_qwen_shapes_mixed_policy(A, N, K, layer, g_expect):
+    """Qwen2.5-7B linear shapes under the R11 mixed policy (g resolved by the
+    library from the layer kind): sampled rows x all columns against the oracle, group sums bit-exact
+    on windows."""
+    M = 320
+    lay = getattr(A, layer)
+    g = A.resolve_group_size(K, 128, A.GRAN_MIXED, lay)
+    assert g == g_expect
+    X, W = inputs.make_gemm_inputs(M, N, K, 7001 + N % 97)
+    qA, sA, ga = A.quantize_act(dev(X), 128, A.GRAN_MIXED, lay)
+    qW, sW, gw = A.pack_weights(dev(W), 128, A.GRAN_MIXED, lay)
+    assert ga == g and gw == g
+    Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, 128, A.GRAN_MIXED, lay).cpu().numpy()
+    rows = inputs.sample_rows(M, 3)
+    qa, sa = O.quantize(X, g)
+    qw, sw = O.quantize(W, g)
+    _, _, codes, _ = gpu_quantize(A, X, g)
+    assert np.array_equal(codes, qa)
+    Y64, T = O.dequant_gemm(qa[rows], sa[rows], qw, sw, g)
+    check_output(Y[rows], Y64, T, K // g, True)
+    for (m0, n0) in [(0, 0), (188, N - 8), (M - 8, 250)]:
+        P = A.debug_group_sums(qA, qW, M, N, K, 128, A.GRAN_MIXED, lay, m0=m0, m1=m0 + 8, n0=n0, n1=n0 + 8).cpu().numpy()
+        assert np.array_equal(P, O.group_sums(qa[m0:m0 + 8], qw[n0:n0 + 8], g))
+
+
 def test_linear_host_matches_device_path(A):
     M, N, K, g = 16, 256, 512, 128
     X, W, _ = inputs.config0()
