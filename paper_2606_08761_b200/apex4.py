@@ -254,7 +254,8 @@ def measure_rho() -> dict:
 
 
 def debug_set_dispatch(nt: int = -1, split: int = -1, grid: int = -1) -> None:
-    """Test hook: force the token-tile width (16..256), stream-K (0/1) and the grid size."""
+    """Test hook: force the kernel / token-tile width (0 = decode kernel, 16..128 = one-CTA tile kernel,
+    256 = CTA pairs, 256 + w = CTA pairs with w = 64 / 128 / 192 tokens per tile), stream-K (0/1) and the grid size."""
     lib().apex4_debug_set_dispatch(nt, split, grid)
 
 

@@ -69,26 +69,39 @@ struct Dispatch {
   int grid;
   int upt, kbu, tiles_m, tiles_n;
   int rows8, mt;   // nt == 0: decode (stream) kernel, 8-row groups per warp and m16 token tiles
+  int pnt;         // nt == 256: tokens per pair tile (64 / 128 / kPairTokens)
 };
 
 // test hook (apex4_debug_set_dispatch): -1 = automatic
-int g_force_nt = -1, g_force_split = -1, g_force_grid = -1;   // g_force_nt == 0 forces the decode kernel
+int g_force_nt = -1, g_force_split = -1, g_force_grid = -1, g_force_pnt = -1;   // g_force_nt == 0 forces the decode kernel
 long long* g_timeline = nullptr;
+
+// Tokens per pair tile: columns past M are wasted epilogue / MMA work, but a 128-token tile costs ~1.2 x
+// a 192-token tile per token (measured at N = K = 8192: M = 1024 146 vs 139 us at g = 128, 88 vs 79 us
+// per-channel; M = 256: 44 vs 54 us).  M <= 64: the 64-token tile.
+int pair_tokens(int M) {
+  if (g_force_pnt > 0) return g_force_pnt;
+  if (M <= 64) return 64;
+  const int r128 = (M + 127) / 128 * 128, r192 = (M + kPairTokens - 1) / kPairTokens * kPairTokens;
+  return 6 * r128 < 5 * r192 ? 128 : kPairTokens;
+}
 
 Dispatch choose_dispatch(int M, int N, int K, int g) {
   Dispatch d;
+  d.pnt = 0;
   const int KB = K / kBlockK;
   d.kbu = g > kBlockK ? g / kBlockK : 1;   // indivisible k unit: a whole group, at least a k-block
   d.upt = KB / d.kbu;
   d.bias = g <= kBlockK;
   d.rows8 = d.mt = 0;
-  const bool gemv_ok = M <= 64 && g == kBlockK;   // larger groups: the tile kernel keeps one rounding per group (R12)
+  // decode kernel: M <= 32 at g = 128 (larger groups need one rounding per group, R12, which it does not
+  // keep; 32 < M <= 64: the pair kernel with 64-token tiles, 24.5 vs 36.2 us at N = K = 8192).  Everything
+  // else runs on CTA pairs; the one-CTA tile kernel (nt = 16..128) and the ring decode kernel are only
+  // reachable through the test hook.
+  const bool gemv_ok = (g_force_nt == 0 ? M <= 64 : M <= 32) && g == kBlockK;
   if (g_force_nt > 0) d.nt = g_force_nt;
   else if (gemv_ok) d.nt = 0;
-  else if (M <= 16) d.nt = 16;
-  else if (M <= 32) d.nt = 32;
-  else if (M <= 64) d.nt = 64;
-  else d.nt = 256;   // the pair kernel also wins for 64 < M <= 128 (40.7 vs 44.0 us at N = K = 8192); nt = 128 only when forced
+  else d.nt = 256;
   if (d.nt == 0) {
     // decode kernel: a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
     d.bias = 0;
@@ -106,7 +119,8 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
     return d;
   }
   const bool pair = d.nt == 256;
-  d.tiles_m = pair ? (M + kPairTokens - 1) / kPairTokens : (M + d.nt - 1) / d.nt;
+  if (pair) d.pnt = pair_tokens(M);
+  d.tiles_m = pair ? (M + d.pnt - 1) / d.pnt : (M + d.nt - 1) / d.nt;
   d.tiles_n = pair ? (N + 2 * kTileRows - 1) / (2 * kTileRows) : (N + kTileRows - 1) / kTileRows;
   const long long tiles = static_cast<long long>(d.tiles_m) * d.tiles_n;
   const long long units = tiles * d.upt;
@@ -138,8 +152,8 @@ cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, c
 }
 size_t workspace_need(const Dispatch& d, int M, int N) {
   if (!d.split) return 0;
-  // pair kernel: every 256 x 192 tile in fragment order (tile-padded); tile kernel: [M, N]
-  if (d.nt == 256) return counters_bytes(d) + static_cast<size_t>(d.tiles_m) * d.tiles_n * 256 * kPairTokens * 4;
+  // pair kernel: every 256 x pnt tile in fragment order (tile-padded); tile kernel: [M, N]
+  if (d.nt == 256) return counters_bytes(d) + static_cast<size_t>(d.tiles_m) * d.tiles_n * 256 * d.pnt * 4;
   return counters_bytes(d) + static_cast<size_t>(M) * N * 4;
 }
 
@@ -257,7 +271,7 @@ static void fill_params(GemmParams& p, const Dispatch& d, const void* qA, const 
   p.qA = static_cast<const uint8_t*>(qA); p.sA = static_cast<const __half*>(sA);
   p.M = M; p.N = N; p.K = K; p.g = g; p.G = K / g;
   p.tiles_m = d.tiles_m; p.tiles_n = d.tiles_n;
-  p.split = d.split; p.upt = d.upt; p.kbu = d.kbu;
+  p.split = d.split; p.upt = d.upt; p.kbu = d.kbu; p.pair_nt = d.pnt;
   p.tl = g_timeline;
 }
 
@@ -360,7 +374,10 @@ int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const 
 // test hooks, not part of the documented ABI: force token-tile width / stream-K / grid size
 // (-1 = automatic).  Process-global; tests restore it.
 int apex4_debug_set_dispatch(int nt, int split, int grid) {
-  g_force_nt = nt; g_force_split = split; g_force_grid = grid;
+  // nt = 256 + w (w = 64 / 128 / 192) forces the pair kernel with w tokens per tile
+  g_force_pnt = (nt > 256) ? nt - 256 : -1;
+  g_force_nt = (nt > 256) ? 256 : nt;
+  g_force_split = split; g_force_grid = grid;
   return APEX4_OK;
 }
 int apex4_debug_set_timeline(void* dev_buf) {

@@ -22,6 +22,7 @@ struct GemmParams {
   // split = 1 -> the K loop of all tiles is one line of `units` dealt to the CTAs in equal contiguous
   // ranges (stream-K); a unit is kbu k-blocks (one group when g >= 128), a tile has upt units.
   int split, upt, kbu;
+  int pair_nt;         // pair kernel: tokens per tile (64 / 128 / kPairTokens)
   float* ws;           // split = 1: FP32 partial sums [M, N], zero on entry, zero on exit
   int* counters;       // split = 1: finished units per tile, zero on entry/exit
   int32_t* P_out;      // debug dump of the per-group INT32 sums (DUMP kernels only)
@@ -33,10 +34,10 @@ struct GemmParams {
 cudaError_t launch_gemm(const GemmParams& p, int nt, bool bias, bool dump, int grid, cudaStream_t st);
 int gemm_max_ctas();   // persistent grid size: one CTA per SM
 
-constexpr int kPairTokens = 192;   // tokens per CTA-pair tile
+constexpr int kPairTokens = 192;   // tokens per CTA-pair tile (the widest; 128 / 64 where M is small)
 
 // Tensor-bound regime (apex4_gemm_pair.cu): CTA pairs (cluster of 2, cta_group::2), work tile = 256
-// weight rows x kPairTokens tokens; tiles_m / tiles_n / counters are in units of pair tiles (counters: two per
+// weight rows x p.pair_nt tokens; tiles_m / tiles_n / counters are in units of pair tiles (counters: two per
 // tile, one per CTA of the pair).  npairs <= gemm_max_pairs().
 cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st);
 int gemm_max_pairs();

@@ -42,32 +42,40 @@ namespace pair {
 constexpr uint32_t kMagicBits = 0x4B400000u;   // float 12582912 = 1.5 * 2^23
 constexpr int kEpiWGs = 2;          // epilogue warpgroups (each owns kNT / kEpiWGs token columns)
 constexpr int kEpiWarps = 4 * kEpiWGs;
-constexpr int kNT = kPairTokens;    // 192 tokens per pair tile = MMA N = accumulator buffer width
-constexpr int kHalf = kNT / 2;      // 96 token rows per CTA (its half of the B operand)
-constexpr int kEpiCols = kNT / kEpiWGs;        // accumulator columns per epilogue warpgroup
-constexpr int kChunks = kEpiCols / 16;         // 16-column TMEM chunks per epilogue thread
 constexpr int kAccBufs = 2;
 constexpr int kOpStages = 4;        // widened operand stages (TMEM A + smem B)
 constexpr int kPkStages = 6;        // packed (bulk copy) stages
 constexpr int kScfSlots = 8;
 constexpr int kTmemA0 = 384;        // first TMEM column of the A-operand stages
 constexpr int kPkWBytes = kBlobBytes;             // 128 weight rows of a k-block
-constexpr int kPkABytes = kHalf * kRowBytes;      // 96 token rows
 constexpr int kPkSWBytes = 4 * 256;               // up to 4 groups per k-block, 128 FP16 each
-constexpr int kPkSABytes = 2 * 4 * 256;           // the two 128-token blobs the tile touches
-constexpr int kPkStageBytes = kPkWBytes + kPkABytes + kPkSWBytes + kPkSABytes;
-constexpr int kI8StageBytes = kHalf * kBlockK;    // widened tokens: [96 rows][128 B]
-constexpr int kScfSlotBytes = kTileRows * 8 + kNT * 4 + 256;   // {a,b} per row, sA per column (padded)
+constexpr int kPkSABytes = 2 * 4 * 256;           // the (up to) two 128-token blobs the tile touches
 constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs;
-constexpr int kStoreBytes = kEpiCols * 64;         // per epilogue warp: [kEpiCols m][32 n] FP16 output staging
-constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
-                           kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + kEpiWarps * kStoreBytes;
 static_assert((kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
 static_assert((kOpStages & (kOpStages - 1)) == 0, "stage index wraps with a mask");
-static_assert(kAccBufs * kNT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
-static_assert(kI8StageBytes % 1024 == 0 && kPkStageBytes % 16 == 0, "alignment");
-static_assert(kSmemBytes <= 232448, "shared memory");
-static_assert(kNT % (16 * kEpiWGs) == 0, "epilogue warpgroups own whole 16-column chunks");
+
+// Everything that depends on the token width NT of the pair tile (MMA N = accumulator buffer width):
+// 192 in the tensor-bound regime, 128 / 64 where M would leave most of a 192-token tile empty.
+template <int NT>
+struct Tile {
+  static constexpr int kNT = NT;
+  static constexpr int kHalf = NT / 2;                  // token rows per CTA (its half of the B operand)
+  static constexpr int kEpiCols = NT / kEpiWGs;         // accumulator columns per epilogue warpgroup
+  static constexpr int kChunks = kEpiCols / 16;         // 16-column TMEM chunks per epilogue thread
+  static constexpr int kTokIters = kHalf / 32;          // 16-byte token pieces per widener thread
+  static constexpr int kPkABytes = kHalf * kRowBytes;   // packed token rows of a k-block
+  static constexpr int kPkStageBytes = kPkWBytes + kPkABytes + kPkSWBytes + kPkSABytes;
+  static constexpr int kI8StageBytes = kHalf * kBlockK; // widened tokens: [kHalf rows][128 B]
+  static constexpr int kScfSlotBytes = kTileRows * 8 + NT * 4 + 256;   // {a,b} per row, sA per column (padded)
+  static constexpr int kStoreBytes = kEpiCols * 64;     // per epilogue warp: [kEpiCols m][32 n] FP16 output staging
+  static constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
+                                    kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + kEpiWarps * kStoreBytes;
+  static_assert(NT % 64 == 0 && NT <= kPairTokens, "token width");
+  static_assert(kAccBufs * NT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
+  static_assert(kI8StageBytes % 1024 == 0 && kPkStageBytes % 16 == 0, "alignment");
+  static_assert(kSmemBytes <= 232448, "shared memory");
+  static_assert(NT % (16 * kEpiWGs) == 0, "epilogue warpgroups own whole 16-column chunks");
+};
 
 // Warp layout for WWG widener warpgroups.  With one, the wideners of a CTA run one k-block at a time:
 // fewer warps polling barriers and competing for issue slots, which is what the epilogue-heavy fine
@@ -98,7 +106,7 @@ inline int widen_wgs(int g) {
 }
 
 struct Work {
-  int nt, mt;      // pair tile: 256 weight rows, 192 tokens
+  int nt, mt;      // pair tile: 256 weight rows x NT tokens
   int kb0, kb1;
   int partial, units;
 };
@@ -138,10 +146,14 @@ __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Wor
 
 using namespace pair;
 
-template <bool BIAS, bool DUMP, int WWG>
+template <bool BIAS, bool DUMP, int WWG, int NT>
 __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
     w4a4_gemm_pair_kernel(const GemmParams p) {
   using L = Warps<WWG>;
+  using T = Tile<NT>;
+  constexpr int kNT = T::kNT, kHalf = T::kHalf, kEpiCols = T::kEpiCols, kChunks = T::kChunks;
+  constexpr int kPkABytes = T::kPkABytes, kPkStageBytes = T::kPkStageBytes, kI8StageBytes = T::kI8StageBytes;
+  constexpr int kScfSlotBytes = T::kScfSlotBytes, kStoreBytes = T::kStoreBytes, kTokIters = T::kTokIters;
   constexpr int kWidenWGs = L::kWidenWGs, kEpiWarp0 = L::kEpiWarp0, kCtlWarp0 = L::kCtlWarp0;
   constexpr int kRegsCtl = L::kRegsCtl, kRegsWiden = L::kRegsWiden, kRegsEpi = L::kRegsEpi;
   extern __shared__ uint8_t smem_raw[];
@@ -235,7 +247,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
         const int n2 = (ab0 + 1 < m_blobs) ? kHalf - min(kHalf, kTileRows - ar0) : 0;
         // token scales: the two blobs the 192-token tile touches
         const int sb0 = (w.mt * kNT) >> 7;
-        const int s_blobs = min(2, m_blobs - sb0);
+        const int s_blobs = min((((w.mt * kNT) & 127) + kNT > kTileRows) ? 2 : 1, m_blobs - sb0);
         const int gfirst0 = g < kBlockK ? w.kb0 * gpk : w.kb0 / kbpg;
         const uint8_t* wsrc = p.qW + wblob * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes;
         const uint8_t* asrc = p.qA + ab0 * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes + ar0 * kRowBytes;
@@ -395,13 +407,13 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
         if (r == 0) stamp(9, kbc);
         // ---- tokens: 96 rows x 4 packed chunks; byte offset o -> INT8 offsets 2o (lo), 2o+16 (hi)
         {
-          uint32_t av[12];
+          uint32_t av[4 * kTokIters];
 #pragma unroll
-          for (int x = 0; x < 3; ++x)
+          for (int x = 0; x < kTokIters; ++x)
             lds128(pk_addr + kPkWBytes + (r + 128 * x) * 16, av[4 * x], av[4 * x + 1], av[4 * x + 2], av[4 * x + 3]);
           const uint32_t dst0 = smem_base + offI8 + t_cur * kI8StageBytes;
 #pragma unroll
-          for (int x = 0; x < 3; ++x) {
+          for (int x = 0; x < kTokIters; ++x) {
             const uint32_t dst = dst0 + (r + 128 * x) * 32;
             const uint32_t l0 = rotl4(av[4 * x]) & kMask, h0 = av[4 * x] & kMask;
             const uint32_t l1 = rotl4(av[4 * x + 1]) & kMask, h1 = av[4 * x + 1] & kMask;
@@ -680,40 +692,49 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <bool BIAS, bool DUMP, int WWG>
+template <bool BIAS, bool DUMP, int WWG, int NT>
 static cudaError_t launch_pair_one(const GemmParams& p, int npairs, cudaStream_t st) {
-  auto kern = w4a4_gemm_pair_kernel<BIAS, DUMP, WWG>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  auto kern = w4a4_gemm_pair_kernel<BIAS, DUMP, WWG, NT>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<NT>::kSmemBytes);
   if (e != cudaSuccess) return e;
-  kern<<<2 * npairs, Warps<WWG>::kThreads, kSmemBytes, st>>>(p);
+  kern<<<2 * npairs, Warps<WWG>::kThreads, Tile<NT>::kSmemBytes, st>>>(p);
   return cudaGetLastError();
 }
-template <int WWG>
+template <int WWG, int NT>
 static cudaError_t launch_pair_w(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
-  if (bias) return dump ? launch_pair_one<true, true, WWG>(p, npairs, st) : launch_pair_one<true, false, WWG>(p, npairs, st);
-  return dump ? launch_pair_one<false, true, WWG>(p, npairs, st) : launch_pair_one<false, false, WWG>(p, npairs, st);
+  if (bias) return dump ? launch_pair_one<true, true, WWG, NT>(p, npairs, st) : launch_pair_one<true, false, WWG, NT>(p, npairs, st);
+  return dump ? launch_pair_one<false, true, WWG, NT>(p, npairs, st) : launch_pair_one<false, false, WWG, NT>(p, npairs, st);
+}
+template <int NT>
+static cudaError_t launch_pair_nt(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
+  return widen_wgs(p.g) == 1 ? launch_pair_w<1, NT>(p, bias, dump, npairs, st) : launch_pair_w<2, NT>(p, bias, dump, npairs, st);
 }
 
 cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
-  return widen_wgs(p.g) == 1 ? launch_pair_w<1>(p, bias, dump, npairs, st) : launch_pair_w<2>(p, bias, dump, npairs, st);
+  switch (p.pair_nt) {
+    case 64: return launch_pair_nt<64>(p, bias, dump, npairs, st);
+    case 128: return launch_pair_nt<128>(p, bias, dump, npairs, st);
+    case kPairTokens: return launch_pair_nt<kPairTokens>(p, bias, dump, npairs, st);
+    default: return cudaErrorInvalidValue;
+  }
 }
 
 // CTA pairs that can be resident at once (one per TPC); queried once
 int gemm_max_pairs() {
   static int pairs = 0;
   if (pairs == 0) {
-    auto kern = w4a4_gemm_pair_kernel<true, false, 2>;   // one CTA per SM whatever the warp layout
+    auto kern = w4a4_gemm_pair_kernel<true, false, 2, kPairTokens>;   // one CTA per SM whatever the layout
     int n = 0;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(2 * 74);
     cfg.blockDim = dim3(Warps<2>::kThreads);
-    cfg.dynamicSmemBytes = kSmemBytes;
+    cfg.dynamicSmemBytes = Tile<kPairTokens>::kSmemBytes;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) != cudaSuccess ||
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<kPairTokens>::kSmemBytes) != cudaSuccess ||
         cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) {
       cudaGetLastError();
       n = gemm_max_ctas() / 2;

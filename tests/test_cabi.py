@@ -80,8 +80,15 @@ def test_dispatch_table(L):
     # decode regime, g = 128: the streaming kernel (nt = 0), 8-row row blocks over all SMs, no workspace
     nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 128)
     assert (nt, split, upt) == (0, 0, 7) and 1 <= grid <= 148
-    assert apex4.debug_get_dispatch(64, 8192, 8192, 128)[0] == 0
+    assert apex4.debug_get_dispatch(32, 8192, 8192, 128)[0] == 0
     assert apex4.workspace_bytes(16, 8192, 8192, 128) == 0
+    # 32 < M <= 64: CTA pairs on 256 x 64 tiles, 32 tiles on <= 74 pairs -> stream-K; workspace = 32 * 2
+    # counters + every 256 x 64 tile as FP32
+    nt, split, grid, upt = apex4.debug_get_dispatch(64, 8192, 8192, 128)
+    assert (nt, split, upt) == (256, 1, 64)
+    assert apex4.workspace_bytes(64, 8192, 8192, 128) == 256 + 32 * 256 * 64 * 4
+    # M = 256: two 128-token tiles instead of a 192-token tile and a third-full one
+    assert apex4.workspace_bytes(256, 4096, 4096, 128) in (0, 256 + 2 * 16 * 256 * 128 * 4)
     # tensor-bound regime: CTA pairs on 256 x 192 tiles; 43 x 32 tiles fill the last wave -> whole tiles
     nt, split, grid, upt = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
     assert (nt, split, upt) == (256, 0, 64) and 1 <= grid <= 74
@@ -91,7 +98,7 @@ def test_dispatch_table(L):
     assert (nt, split, upt) == (256, 1, 32)
     # 11 * 16 * 2 counters (padded to 256 bytes) + every 256 x 192 tile as FP32 in fragment order
     assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 11 * 16 * 256 * 192 * 4
-    # per-channel at small M: the tile kernel; the k range cannot be split inside a group
+    # per-channel at small M: CTA pairs on 256 x 64 tiles; the k range cannot be split inside a group
     nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
-    assert (nt, split, grid, upt) == (16, 0, 64, 1)
+    assert (nt, split, grid, upt) == (256, 0, 32, 1)
     assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0

@@ -167,17 +167,30 @@ def test_gemm_ragged_and_multi_tile(A, M, N, K, g):
                                    (33, 264, 2048), (48, 520, 1024), (64, 456, 1536), (5, 64, 28672)])
 @pytest.mark.parametrize("grid", [-1, 1, 3])
 def test_gemm_decode_kernels(A, M, N, K, grid):
-    """The decode-regime kernels (M <= 64, g = 128: bulk-copy staged for one or two m16 token tiles,
-    register-ring for three or four) on ragged N, row ranges that straddle 128-row tiles, K from one
-    k-block to the longest supported row, and several grid sizes (rows per CTA / batches per CTA)."""
-    assert A.debug_get_dispatch(M, N, K, 128)[0] == 0          # automatic dispatch picks the decode kernel
+    """The decode-regime kernels (g = 128: bulk-copy staged for one or two m16 token tiles -- the automatic
+    choice for M <= 32 --, register-ring for three or four, reachable through the test hook) on ragged N,
+    row ranges that straddle 128-row tiles, K from one k-block to the longest supported row, and several
+    grid sizes (rows per CTA / batches per CTA)."""
+    # automatic dispatch: the decode kernel up to M = 32, CTA pairs on 64-token tiles above
+    assert A.debug_get_dispatch(M, N, K, 128)[0] == (0 if M <= 32 else 256)
     run_gemm_case(A, M, N, K, 128, seed=300 + M, dispatch=(0, -1, grid))
+
+
+@pytest.mark.parametrize("M,N,K,g", [(40, 264, 512, 128), (64, 520, 1024, 32), (100, 520, 1024, 128),
+                                     (130, 304, 1024, 512), (300, 520, 1024, 1024), (200, 264, 2048, 64)])
+@pytest.mark.parametrize("dispatch", [(256 + 64, 0, -1), (256 + 128, 0, -1), (256 + 192, 0, -1),
+                                      (256 + 64, 1, 3), (256 + 128, 1, 5)])
+def test_gemm_pair_tile_widths(A, M, N, K, g, dispatch):
+    """The CTA-pair kernel at its three token-tile widths (64 / 128 / 192; the hook value is 256 + width),
+    whole tiles and stream-K, FP16 and FP32 output, on ragged shapes."""
+    run_gemm_case(A, M, N, K, g, seed=500 + M, dispatch=dispatch)
+    run_gemm_case(A, M, N, K, g, seed=500 + M, dispatch=dispatch, out_f32=True, sums=None)
 
 
 def test_gemm_decode_f32_and_large_group_routing(A):
     run_gemm_case(A, 16, 256, 1024, 128, seed=7, out_f32=True, dispatch=(0, -1, -1))
-    # groups larger than a k-block keep one rounding per group: the tile kernel handles them
-    assert A.debug_get_dispatch(16, 256, 1024, 256)[0] != 0
+    # groups larger than a k-block keep one rounding per group: the pair kernel handles them
+    assert A.debug_get_dispatch(16, 256, 1024, 256)[0] == 256
     run_gemm_case(A, 16, 256, 1024, 256, seed=8)
 
 
