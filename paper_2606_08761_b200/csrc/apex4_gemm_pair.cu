@@ -1,7 +1,8 @@
-// apex4_gemm_pair.cu -- a2..a7 of the hot path for the tensor-bound regime (M > 128): the W4A4
+// apex4_gemm_pair.cu -- a2..a7 of the hot path (every shape but decode M <= 32 at g = 128): the W4A4
 // group-dequant GEMM of Eq. 8 on a CTA PAIR (cluster of 2, tcgen05 cta_group::2).
 //
-// A pair owns a 256 (weight rows n) x 192 (tokens m) output tile.  CTA r of the pair holds weight
+// A pair owns a 256 (weight rows n) x NT (tokens m) output tile; NT = 192 below, 128 / 64 are the same
+// kernel instantiated for small M (Tile<NT>).  CTA r of the pair holds weight
 // rows 128 r .. 128 r + 127 of the tile on its 128 TMEM lanes and supplies 96 of the 192 token rows
 // of every MMA from its own shared memory, so per SM and k-block (K = 128) only 8 KB of packed
 // weights and 6 KB of packed activations are fetched, widened and read by the tensor core
