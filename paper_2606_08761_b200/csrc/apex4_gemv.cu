@@ -97,7 +97,9 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
   constexpr uint32_t offStage = Cfg::kPartBytes;
   constexpr uint32_t offBar = offStage + kWarps * kStages * Cfg::kStageBytes;
 
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  // warp index through a shuffle: tells the compiler it is warp-uniform, so the copy descriptors of
+  // issue_next live in uniform registers (per-thread operands cost an R2UR waterfall per UBLKCP)
+  const int lane = threadIdx.x & 31, w = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
   const int q = lane >> 2, t = lane & 3;
   const int KB = p.K / kBlockK;
   const int kbw0 = KB * w / kWarps, kbw1 = KB * (w + 1) / kWarps;    // this warp's k-blocks
@@ -116,9 +118,13 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
   }
   __syncwarp();
 
-  // ---- issue cursor: (batch start row block, k-block index of this warp), flattened, k fastest
+  // ---- issue cursor: (batch start row block, k-block index of this warp), flattened, k fastest.
+  // The whole warp runs the bookkeeping on warp-uniform values and one elected lane issues: with the
+  // cursor private to lane 0 the divergent block cost the warp ~185 issue slots per k-block (a third
+  // of the loop), every copy sitting in an R2UR / BRA.U.ANY waterfall.
+  const bool el = elect_one();
   int ib0 = rb0, ij = 0, islot = 0;
-  auto issue_next = [&]() {                             // elected lane: copies of one stage
+  auto issue_next = [&]() {                             // copies of one stage
     if (ib0 >= rb1 || nkw == 0) return;
     const int nb = min(RBB, rb1 - ib0);
     const int kb = kbw0 + ij;
@@ -128,7 +134,8 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     const int tile_a = row_a >> 7;
     const int split_row = min(row_b, (tile_a + 1) << 7);               // rows [row_a, split_row) in tile_a
     const int n1 = split_row - row_a, n2 = row_b - split_row;
-    const int gm = kb / p.kbu;
+    const int gm = p.kbu == 1 ? kb : kb / p.kbu;        // dispatch only sends g = 128 here (kbu = 1)
+    if (el) {
     mbar_arrive_expect_tx(full, (n1 + n2) * kRowBytes + Cfg::kABytes + (n1 + n2) * 2 + Cfg::kSABytes);
     bulk_g2s(st, p.qW + tile_a * row_pitch + static_cast<size_t>(kb) * kBlobBytes + (row_a & 127) * kRowBytes,
              n1 * kRowBytes, full);
@@ -143,11 +150,11 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     bulk_g2s(st + Cfg::kWBytes, p.qA + static_cast<size_t>(kb) * kBlobBytes, Cfg::kABytes, full);
     bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, p.sA + static_cast<size_t>(gm) * kTileRows,
              Cfg::kSABytes, full);
+    }
     islot = islot + 1 == kStages ? 0 : islot + 1;
     if (++ij == nkw) { ij = 0; ib0 += RBB; }
   };
-  if (lane == 0)
-    for (int s = 0; s < kStages; ++s) issue_next();
+  for (int s = 0; s < kStages; ++s) issue_next();
 
   uint32_t par = 0;                                     // phase parity of the warp's stage barriers
   int cslot = 0;
@@ -223,7 +230,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
         }
       }
       __syncwarp();                                     // every lane is done reading the stage
-      if (lane == 0) issue_next();                      // re-arm it with the warp's next k-block
+      issue_next();                                     // re-arm it with the warp's next k-block
       cslot = cslot + 1 == kStages ? 0 : cslot + 1;
     }
 
