@@ -123,36 +123,53 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
   // cursor private to lane 0 the divergent block cost the warp ~185 issue slots per k-block (a third
   // of the loop), every copy sitting in an R2UR / BRA.U.ANY waterfall.
   const bool el = elect_one();
+  // Source pointers advance by a blob (k-block) per stage and are set up once per batch: recomputing them
+  // per stage cost ~120 (uniform-datapath) instructions per k-block.  One group per k-block (g = 128, the
+  // only granularity the dispatcher sends here): group index = k-block index.
   int ib0 = rb0, ij = 0, islot = 0;
-  auto issue_next = [&]() {                             // copies of one stage
-    if (ib0 >= rb1 || nkw == 0) return;
+  const uint8_t *w1 = nullptr, *w2 = nullptr, *aq = nullptr;
+  const __half *s1 = nullptr, *s2 = nullptr, *sq = nullptr;
+  uint32_t n1b = 0, n2b = 0, tx = 0;                    // rows x 64 bytes of the two pieces, bytes per stage
+  auto batch_setup = [&]() {
     const int nb = min(RBB, rb1 - ib0);
-    const int kb = kbw0 + ij;
-    const uint32_t st = my_stage0 + islot * Cfg::kStageBytes;
-    const uint32_t full = my_bar0 + 8 * islot;
     const int row_a = ib0 * 8, row_b = row_a + nb * 8;                 // weight rows of the batch
     const int tile_a = row_a >> 7;
     const int split_row = min(row_b, (tile_a + 1) << 7);               // rows [row_a, split_row) in tile_a
     const int n1 = split_row - row_a, n2 = row_b - split_row;
-    const int gm = p.kbu == 1 ? kb : kb / p.kbu;        // dispatch only sends g = 128 here (kbu = 1)
+    w1 = p.qW + tile_a * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes + (row_a & 127) * kRowBytes;
+    w2 = p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes;
+    s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + kbw0) * kTileRows + (row_a & 127);
+    s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + kbw0) * kTileRows;
+    aq = p.qA + static_cast<size_t>(kbw0) * kBlobBytes;
+    sq = p.sA + static_cast<size_t>(kbw0) * kTileRows;
+    n1b = n1 * kRowBytes;
+    n2b = n2 * kRowBytes;
+    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + (n1 + n2) * 2 + Cfg::kSABytes;
+  };
+  if (rb0 < rb1 && nkw > 0) batch_setup();
+  auto issue_next = [&]() {                             // copies of one stage
+    if (ib0 >= rb1 || nkw == 0) return;
+    const uint32_t st = my_stage0 + islot * Cfg::kStageBytes;
+    const uint32_t full = my_bar0 + 8 * islot;
     if (el) {
-    mbar_arrive_expect_tx(full, (n1 + n2) * kRowBytes + Cfg::kABytes + (n1 + n2) * 2 + Cfg::kSABytes);
-    bulk_g2s(st, p.qW + tile_a * row_pitch + static_cast<size_t>(kb) * kBlobBytes + (row_a & 127) * kRowBytes,
-             n1 * kRowBytes, full);
-    bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes,
-             p.sW + (static_cast<size_t>(tile_a) * p.G + gm) * kTileRows + (row_a & 127), n1 * 2, full);
-    if (n2 > 0) {
-      bulk_g2s(st + n1 * kRowBytes, p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kb) * kBlobBytes,
-               n2 * kRowBytes, full);
-      bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + n1 * 2,
-               p.sW + (static_cast<size_t>(tile_a + 1) * p.G + gm) * kTileRows, n2 * 2, full);
+      mbar_arrive_expect_tx(full, tx);
+      bulk_g2s(st, w1, n1b, full);
+      bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes, s1, n1b >> 5, full);   // 2 bytes per row
+      if (n2b > 0) {
+        bulk_g2s(st + n1b, w2, n2b, full);
+        bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + (n1b >> 5), s2, n2b >> 5, full);
+      }
+      bulk_g2s(st + Cfg::kWBytes, aq, Cfg::kABytes, full);
+      bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, sq, Cfg::kSABytes, full);
     }
-    bulk_g2s(st + Cfg::kWBytes, p.qA + static_cast<size_t>(kb) * kBlobBytes, Cfg::kABytes, full);
-    bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, p.sA + static_cast<size_t>(gm) * kTileRows,
-             Cfg::kSABytes, full);
-    }
+    w1 += kBlobBytes; w2 += kBlobBytes; aq += kBlobBytes;
+    s1 += kTileRows; s2 += kTileRows; sq += kTileRows;
     islot = islot + 1 == kStages ? 0 : islot + 1;
-    if (++ij == nkw) { ij = 0; ib0 += RBB; }
+    if (++ij == nkw) {
+      ij = 0;
+      ib0 += RBB;
+      if (ib0 < rb1) batch_setup();
+    }
   };
   for (int s = 0; s < kStages; ++s) issue_next();
 
@@ -276,6 +293,7 @@ template <int MT>
 static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaStream_t st) {
   constexpr int smem = GemvCfg<MT>::kSmemBytes;
   cudaError_t e;
+  if (p.kbu != 1) return cudaErrorInvalidValue;   // one group per k-block (g = 128): see issue_next
   if (dump) {
     auto kern = w4a4_gemv_kernel<MT, true>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
