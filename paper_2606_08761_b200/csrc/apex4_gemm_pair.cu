@@ -123,6 +123,9 @@ __device__ __forceinline__ void work_begin(const GemmParams& p, WorkIter& it, in
 }
 // Tiles are numbered token-tile fastest: pairs that run together share weight tiles in L2.
 __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Work& w, int cp, int npairs) {
+#ifdef APEX4_PAIR_EMPTY   // tuning builds only: launch + set-up + teardown cost
+  return false;
+#endif
   int tile;
   if (p.split == 0) {
     tile = cp + it.i * npairs;
