@@ -86,7 +86,11 @@ struct GemvCfg {
   static_assert(kStageBytes % 16 == 0 && kSmemBytes <= 232448, "shared memory");
 };
 
-template <int MT, bool DUMP>
+// CH: per-channel (one group = all of K).  The warps' k ranges are then parts of ONE group, so the
+// partial sums stay INT32 through the k loop and through the cross-warp reduction (exact), and the two
+// scales are applied once at the end -- one rounding per group as R12 wants, which the per-k-block FP32
+// scaling of the g = 128 path cannot give for larger groups.  |256 P| <= 2^8 * 64 * 32768 = 2^29: no overflow.
+template <int MT, bool DUMP, bool CH>
 __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams p) {
   using Cfg = GemvCfg<MT>;
   constexpr int RBB = Cfg::RBB;
@@ -138,13 +142,15 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     const int n1 = split_row - row_a, n2 = row_b - split_row;
     w1 = p.qW + tile_a * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes + (row_a & 127) * kRowBytes;
     w2 = p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes;
-    s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + kbw0) * kTileRows + (row_a & 127);
-    s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + kbw0) * kTileRows;
+    if constexpr (!CH) {
+      s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + kbw0) * kTileRows + (row_a & 127);
+      s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + kbw0) * kTileRows;
+      sq = p.sA + static_cast<size_t>(kbw0) * kTileRows;
+    }
     aq = p.qA + static_cast<size_t>(kbw0) * kBlobBytes;
-    sq = p.sA + static_cast<size_t>(kbw0) * kTileRows;
     n1b = n1 * kRowBytes;
     n2b = n2 * kRowBytes;
-    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + (n1 + n2) * 2 + Cfg::kSABytes;
+    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + (CH ? 0 : (n1 + n2) * 2 + Cfg::kSABytes);
   };
   if (rb0 < rb1 && nkw > 0) batch_setup();
   auto issue_next = [&]() {                             // copies of one stage
@@ -154,13 +160,13 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     if (el) {
       mbar_arrive_expect_tx(full, tx);
       bulk_g2s(st, w1, n1b, full);
-      bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes, s1, n1b >> 5, full);   // 2 bytes per row
+      if constexpr (!CH) bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes, s1, n1b >> 5, full);   // 2 bytes per row
       if (n2b > 0) {
         bulk_g2s(st + n1b, w2, n2b, full);
-        bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + (n1b >> 5), s2, n2b >> 5, full);
+        if constexpr (!CH) bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + (n1b >> 5), s2, n2b >> 5, full);
       }
       bulk_g2s(st + Cfg::kWBytes, aq, Cfg::kABytes, full);
-      bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, sq, Cfg::kSABytes, full);
+      if constexpr (!CH) bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, sq, Cfg::kSABytes, full);
     }
     w1 += kBlobBytes; w2 += kBlobBytes; aq += kBlobBytes;
     s1 += kTileRows; s2 += kTileRows; sq += kTileRows;
@@ -184,6 +190,13 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       for (int mi = 0; mi < MT; ++mi)
 #pragma unroll
         for (int e = 0; e < 4; ++e) yf[i][mi][e] = 0.f;
+    int ia[RBB][MT][4];                                 // CH: 256 x the INT32 sums over this warp's k range
+#pragma unroll
+    for (int i = 0; i < RBB; ++i)
+#pragma unroll
+      for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) ia[i][mi][e] = 0;
 
     for (int j = 0; j < nkw; ++j) {
       const uint32_t st = my_stage0 + cslot * Cfg::kStageBytes;
@@ -204,9 +217,11 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
           af[mi][i][0] = swap ? h0 : l0; af[mi][i][2] = swap ? l0 : h0;   // token q: k lo / hi half
           af[mi][i][1] = swap ? h1 : l1; af[mi][i][3] = swap ? l1 : h1;   // token q + 8
         }
-        const __half* sah = reinterpret_cast<const __half*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes);
-        sa[mi][0] = __half2float(sah[16 * mi + q]);
-        sa[mi][1] = __half2float(sah[16 * mi + q + 8]);
+        if constexpr (!CH) {
+          const __half* sah = reinterpret_cast<const __half*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes);
+          sa[mi][0] = __half2float(sah[16 * mi + q]);
+          sa[mi][1] = __half2float(sah[16 * mi + q + 8]);
+        }
       }
       const int gm = DUMP ? (kbw0 + j) / p.kbu : 0;
 #pragma unroll
@@ -214,6 +229,15 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
         if (i < nb) {
           uint32_t x[4];
           lds128(st + i * 512 + lane_off, x[0], x[1], x[2], x[3]);
+          if constexpr (CH) {
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4) {
+              const uint32_t b0w = rotl4(x[k4]) & kMask, b1w = x[k4] & kMask;
+#pragma unroll
+              for (int mi = 0; mi < MT; ++mi) mma_s8(ia[i][mi], af[mi][k4], b0w, b1w);
+            }
+            continue;
+          }
           const __half2 sw2 = *reinterpret_cast<const __half2*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + i * 16 + 4 * t);
           int acc[MT][4];
 #pragma unroll
@@ -256,21 +280,49 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     for (int i = 0; i < RBB; ++i)
 #pragma unroll
       for (int mi = 0; mi < MT; ++mi)
-        part[((i * kWarps + w) * MT + mi) * 32 + lane] = make_float4(yf[i][mi][0], yf[i][mi][1], yf[i][mi][2], yf[i][mi][3]);
+        part[((i * kWarps + w) * MT + mi) * 32 + lane] =
+            CH ? make_float4(__int_as_float(ia[i][mi][0]), __int_as_float(ia[i][mi][1]), __int_as_float(ia[i][mi][2]),
+                             __int_as_float(ia[i][mi][3]))
+               : make_float4(yf[i][mi][0], yf[i][mi][1], yf[i][mi][2], yf[i][mi][3]);
     __syncthreads();
-    if (p.Y != nullptr) {
+    if (p.Y != nullptr || (CH && DUMP)) {
       for (int i = w; i < nb; i += kWarps) {
 #pragma unroll
         for (int mi = 0; mi < MT; ++mi) {
           float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+          const int n = (b0 + i) * 8 + 2 * t;
+          const int m = 16 * mi + q;
+          if constexpr (CH) {
+            int s0 = 0, s1i = 0, s2i = 0, s3 = 0;         // exact: INT32 all the way
+#pragma unroll
+            for (int ww = 0; ww < kWarps; ++ww) {
+              const float4 xx = part[((i * kWarps + ww) * MT + mi) * 32 + lane];
+              s0 += __float_as_int(xx.x); s1i += __float_as_int(xx.y); s2i += __float_as_int(xx.z); s3 += __float_as_int(xx.w);
+            }
+            s0 >>= 8; s1i >>= 8; s2i >>= 8; s3 >>= 8;       // operands were 16 q each
+            if constexpr (DUMP) {
+              const int sums[4] = {s0, s1i, s2i, s3};
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const int mm = m + 8 * (e >> 1), nn = n + (e & 1);
+                if (mm >= p.pm0 && mm < p.pm1 && nn >= p.pn0 && nn < p.pn1)
+                  p.P_out[(static_cast<size_t>(mm - p.pm0) * (p.pn1 - p.pn0) + (nn - p.pn0)) * p.G] = sums[e];
+              }
+            }
+            if (p.Y == nullptr || n >= p.N) continue;
+            // one group: Y = float(P) sW sA (a5), P exact in FP32 (|P| <= 64 K < 2^24)
+            const float sw0 = __half2float(__ldg(p.sW + st16_index(n, 0, 1))), sw1 = __half2float(__ldg(p.sW + st16_index(n + 1, 0, 1)));
+            const float sa0 = __half2float(__ldg(p.sA + st16_index(m, 0, 1))), sa1 = __half2float(__ldg(p.sA + st16_index(m + 8, 0, 1)));
+            v.x = __int2float_rn(s0) * sw0 * sa0; v.y = __int2float_rn(s1i) * sw1 * sa0;
+            v.z = __int2float_rn(s2i) * sw0 * sa1; v.w = __int2float_rn(s3) * sw1 * sa1;
+          } else {
 #pragma unroll
           for (int ww = 0; ww < kWarps; ++ww) {
             const float4 xx = part[((i * kWarps + ww) * MT + mi) * 32 + lane];
             v.x += xx.x; v.y += xx.y; v.z += xx.z; v.w += xx.w;
           }
-          const int n = (b0 + i) * 8 + 2 * t;
-          const int m = 16 * mi + q;
-          if (n < p.N) {
+          }
+          if (p.Y != nullptr && n < p.N) {
             if (p.out_f32) {
               float* y = static_cast<float*>(p.Y);
               if (m < p.M) *reinterpret_cast<float2*>(y + static_cast<size_t>(m) * p.N + n) = make_float2(v.x, v.y);
@@ -289,17 +341,16 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <int MT>
+template <int MT, bool CH>
 static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaStream_t st) {
   constexpr int smem = GemvCfg<MT>::kSmemBytes;
   cudaError_t e;
-  if (p.kbu != 1) return cudaErrorInvalidValue;   // one group per k-block (g = 128): see issue_next
   if (dump) {
-    auto kern = w4a4_gemv_kernel<MT, true>;
+    auto kern = w4a4_gemv_kernel<MT, true, CH>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     kern<<<grid, kThreads, smem, st>>>(p);
   } else {
-    auto kern = w4a4_gemv_kernel<MT, false>;
+    auto kern = w4a4_gemv_kernel<MT, false, CH>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     kern<<<grid, kThreads, smem, st>>>(p);
   }
@@ -308,9 +359,12 @@ static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaS
 
 // mt: m16 token tiles (1 or 2; apex4_gemv_ring.cu takes 3 and 4)
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st) {
+  // one group per k-block (g = 128), or one group for all of K (per-channel, exact INT32 reduction)
+  const bool ch = p.G == 1 && p.K > kBlockK;
+  if (!ch && p.kbu != 1) return cudaErrorInvalidValue;
   switch (mt) {
-    case 1: return launch_gemv_m<1>(p, dump, grid, st);
-    case 2: return launch_gemv_m<2>(p, dump, grid, st);
+    case 1: return ch ? launch_gemv_m<1, true>(p, dump, grid, st) : launch_gemv_m<1, false>(p, dump, grid, st);
+    case 2: return ch ? launch_gemv_m<2, true>(p, dump, grid, st) : launch_gemv_m<2, false>(p, dump, grid, st);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -98,7 +98,9 @@ def test_dispatch_table(L):
     assert (nt, split, upt) == (256, 1, 32)
     # 11 * 16 * 2 counters (padded to 256 bytes) + every 256 x 192 tile as FP32 in fragment order
     assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 11 * 16 * 256 * 192 * 4
-    # per-channel at small M: CTA pairs on 256 x 64 tiles; the k range cannot be split inside a group
-    nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 8192)
-    assert (nt, split, grid, upt) == (256, 0, 32, 1)
+    # per-channel decode: the streaming kernel with an exact INT32 cross-warp reduction, no workspace
+    assert apex4.debug_get_dispatch(16, 8192, 8192, 8192)[:2] == (0, 0)
+    # groups between 128 and K at small M: CTA pairs on 256 x 64 tiles; a group is the indivisible k unit
+    nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 1024)
+    assert (nt, upt) == (256, 8)
     assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0

@@ -176,6 +176,17 @@ def test_gemm_decode_kernels(A, M, N, K, grid):
     run_gemm_case(A, M, N, K, 128, seed=300 + M, dispatch=(0, -1, grid))
 
 
+@pytest.mark.parametrize("M,N,K", [(1, 8, 256), (16, 136, 1024), (17, 1000, 512), (32, 8192, 256),
+                                   (20, 264, 2048), (5, 64, 28672)])
+@pytest.mark.parametrize("grid", [-1, 1, 3])
+def test_gemm_decode_per_channel(A, M, N, K, grid):
+    """Per-channel decode (M <= 32, g = K): the decode kernel keeps INT32 partial sums through the k loop
+    and the cross-warp reduction, so the group sum is exact and rounded once (R12)."""
+    assert A.debug_get_dispatch(M, N, K, K)[0] == 0
+    run_gemm_case(A, M, N, K, K, seed=700 + M, dispatch=(0, -1, grid))
+    run_gemm_case(A, M, N, K, K, seed=700 + M, dispatch=(0, -1, grid), out_f32=True, sums=None)
+
+
 @pytest.mark.parametrize("M,N,K,g", [(40, 264, 512, 128), (64, 520, 1024, 32), (100, 520, 1024, 128),
                                      (130, 304, 1024, 512), (300, 520, 1024, 1024), (200, 264, 2048, 64)])
 @pytest.mark.parametrize("dispatch", [(256 + 64, 0, -1), (256 + 128, 0, -1), (256 + 192, 0, -1),
