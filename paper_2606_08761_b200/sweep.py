@@ -194,7 +194,7 @@ def run_sweeps(dev, peaks=None):
         "baseline_mix_fine128_us": round((2 * t[128] + 5 * t[8192]) / 7, 2),
         "uniform_g128_us": t[128]}
     res["config4_llama70b"] = cfg4
-    res["block_policies"] = run_block_policies(dev)
+    res["block_policies"] = run_block_policies(dev, 2048) + run_block_policies(dev, 16)   # prefill and decode
     f11 = {(jobs[i][1], jobs[i][4]): done[i] for i in range(len(jobs)) if jobs[i][0] == "fig11"}
     res["fig11_g128_over_channel"] = [
         {"M": M, "g128_us": f11[(M, 128)]["us"], "channel_us": f11[(M, 8192)]["us"],
