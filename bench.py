@@ -103,9 +103,13 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "window": window}
 
 
-def oracle_sample(sample_rows):
+CPU_BASELINE_ROWS = 1024     # about 10-15 s of oracle time on the GPU box's host cores
+
+
+def oracle_sample(sample_rows, chunk=64):
     """The oracle as it stands on a bounded sample of the workload: the first `sample_rows` token rows
-    of every config-1 layer (activation quantizer + full-width Eq. 8 against the whole weight)."""
+    of every config-1 layer (activation quantizer + full-width Eq. 8 against the whole weight), called on
+    `chunk` rows at a time (its per-group INT sums of all rows at once would not fit in host memory)."""
     import threadpoolctl
     from oracle import apex4_oracle as O
     from paper_2606_08761_b200 import inputs
@@ -116,8 +120,9 @@ def oracle_sample(sample_rows):
         W = inputs.make_weights(n, k, seed)
         qW, sW = O.quantize(W, G)          # offline (a0): not timed, as on the GPU side
         t0 = time.perf_counter()
-        qA, sA = O.quantize(X, G)
-        Y = O.to_f16(O.dequant_gemm(qA, sA, qW, sW, G, want_T=False))
+        for r0 in range(0, sample_rows, chunk):
+            qA, sA = O.quantize(X[r0:r0 + chunk], G)
+            Y = O.to_f16(O.dequant_gemm(qA, sA, qW, sW, G, want_T=False))
         secs += time.perf_counter() - t0
         ops += 2.0 * sample_rows * n * k
         del W, qW, sW, Y
@@ -302,9 +307,9 @@ def main():
         "roofline": roofline,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, secs, cores = oracle_sample(32)
+        v, secs, cores = oracle_sample(CPU_BASELINE_ROWS)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                               "sample": f"first 32 of {M_PREFILL} token rows of each layer, full N and K "
+                               "sample": f"first {CPU_BASELINE_ROWS} of {M_PREFILL} token rows of each layer, full N and K "
                                          f"({secs:.1f} s of numpy float64 oracle)"}
     if args.sweep and rank == 0:
         from paper_2606_08761_b200 import sweep
