@@ -103,7 +103,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "window": window}
 
 
-CPU_BASELINE_ROWS = 1024     # about 10-15 s of oracle time on the GPU box's host cores
+CPU_BASELINE_ROWS = 2048     # all token rows of every layer: about 15 s of oracle time on the GPU box (16 cores)
 
 
 def oracle_sample(sample_rows, chunk=64):
