@@ -83,7 +83,7 @@ size_t apex4_packed_bytes(int R, int K);
 /* Number of FP16 elements of the ST16 scale buffer for R rows at resolved group size g. */
 size_t apex4_scale_elems(int R, int K, int g);
 /* Bytes of DEVICE workspace apex4_w4a4_gemm needs for this problem.  0 when every output tile is
- * computed by one CTA (pair) alone: the decode kernels (M <= 32 at g = 128 or per-channel) and any tile count that
+ * computed by one CTA (pair) alone: the decode kernels (M <= 32 at g <= 128 or per-channel) and any tile count that
  * fills the SMs evenly.  Otherwise (stream-K, a6) it holds the tile arrival counters followed by the
  * FP32 partial sums of the shared tiles (padded to whole tiles).  The workspace must be zero-filled
  * once by the caller before its first use; every call leaves it zero-filled again, so one buffer

@@ -94,12 +94,13 @@ Dispatch choose_dispatch(int M, int N, int K, int g) {
   d.upt = KB / d.kbu;
   d.bias = g <= kBlockK;
   d.rows8 = d.mt = 0;
-  // decode kernel: M <= 32 at g = 128 or per-channel (groups in between need one rounding per group, R12,
+  // decode kernel: M <= 32 at g = 32 / 64 / 128 or per-channel (groups in between need one rounding per group, R12,
   // which its per-k-block FP32 scaling does not keep; 32 < M <= 64: the pair kernel with 64-token tiles, 24.5 vs 36.2 us at N = K = 8192).  Everything
   // else runs on CTA pairs; the one-CTA tile kernel (nt = 16..128) and the ring decode kernel are only
   // reachable through the test hook.
   // per-channel (g = K): the same decode kernel with an exact INT32 cross-warp reduction (M <= 32)
-  const bool gemv_ok = ((g_force_nt == 0 ? M <= 64 : M <= 32) && g == kBlockK) || (M <= 32 && g == K && K > kBlockK);
+  const bool gemv_ok = ((g_force_nt == 0 ? M <= 64 : M <= 32) && g == kBlockK) || (M <= 32 && g == K && K > kBlockK) ||
+                       (M <= 32 && (g == 32 || g == 64));   // fine groups: one MMA (pair) per group
   if (g_force_nt > 0) d.nt = g_force_nt;
   else if (gemv_ok) d.nt = 0;
   else d.nt = 256;

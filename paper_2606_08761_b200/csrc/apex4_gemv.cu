@@ -73,13 +73,14 @@ using namespace gemv;
 
 
 // MT: m16 token tiles (M <= 16 MT).  p.tiles_n = 8-row row blocks; p.kbu = k-blocks per group.
-template <int MT>
+// GS: groups per k-block (1: g >= 128; 2: g = 64; 4: g = 32)
+template <int MT, int GS = 1>
 struct GemvCfg {
   static constexpr int RBB = MT == 1 ? 7 : MT == 2 ? 4 : MT == 3 ? 2 : 1;         // row blocks per batch
   static constexpr int kWBytes = RBB * 8 * kRowBytes;                // weight rows of a k-block
   static constexpr int kABytes = MT * 16 * kRowBytes;                // token rows of a k-block
-  static constexpr int kSWBytes = (RBB * 16 + 15) / 16 * 16;         // FP16 weight scales of the batch rows
-  static constexpr int kSABytes = MT * 32;                           // FP16 token scales
+  static constexpr int kSWBytes = RBB * 16 * GS;                     // FP16 weight scales of the batch rows, [group][row]
+  static constexpr int kSABytes = MT * 32 * GS;                      // FP16 token scales, [group][token]
   static constexpr int kStageBytes = kWBytes + kABytes + kSWBytes + kSABytes;
   static constexpr int kPartBytes = RBB * kWarps * MT * 512;         // FP32 partial sums of a batch
   static constexpr int kSmemBytes = 128 + kPartBytes + kWarps * kStages * kStageBytes + kWarps * kStages * 8;
@@ -90,9 +91,13 @@ struct GemvCfg {
 // partial sums stay INT32 through the k loop and through the cross-warp reduction (exact), and the two
 // scales are applied once at the end -- one rounding per group as R12 wants, which the per-k-block FP32
 // scaling of the g = 128 path cannot give for larger groups.  |256 P| <= 2^8 * 64 * 32768 = 2^29: no overflow.
-template <int MT, bool DUMP, bool CH>
+// GS > 1 (g = 64 / 32): lane (q, t) takes word t of each of the row's four 16-byte chunks instead of chunk t,
+// so that MMA c covers exactly k = 32 c .. 32 c + 31 of the k-block, i.e. one g = 32 group (half a g = 64
+// group), and every group gets its own scales.
+template <int MT, bool DUMP, bool CH, int GS>
 __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams p) {
-  using Cfg = GemvCfg<MT>;
+  static_assert(!(CH && GS > 1), "per-channel has one group");
+  using Cfg = GemvCfg<MT, GS>;
   constexpr int RBB = Cfg::RBB;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
@@ -143,14 +148,14 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     w1 = p.qW + tile_a * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes + (row_a & 127) * kRowBytes;
     w2 = p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes;
     if constexpr (!CH) {
-      s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + kbw0) * kTileRows + (row_a & 127);
-      s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + kbw0) * kTileRows;
-      sq = p.sA + static_cast<size_t>(kbw0) * kTileRows;
+      s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + GS * kbw0) * kTileRows + (row_a & 127);
+      s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + GS * kbw0) * kTileRows;
+      sq = p.sA + static_cast<size_t>(GS * kbw0) * kTileRows;
     }
     aq = p.qA + static_cast<size_t>(kbw0) * kBlobBytes;
     n1b = n1 * kRowBytes;
     n2b = n2 * kRowBytes;
-    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + (CH ? 0 : (n1 + n2) * 2 + Cfg::kSABytes);
+    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + (CH ? 0 : GS * (n1 + n2) * 2 + Cfg::kSABytes);
   };
   if (rb0 < rb1 && nkw > 0) batch_setup();
   auto issue_next = [&]() {                             // copies of one stage
@@ -160,16 +165,20 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     if (el) {
       mbar_arrive_expect_tx(full, tx);
       bulk_g2s(st, w1, n1b, full);
-      if constexpr (!CH) bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes, s1, n1b >> 5, full);   // 2 bytes per row
-      if (n2b > 0) {
-        bulk_g2s(st + n1b, w2, n2b, full);
-        if constexpr (!CH) bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + (n1b >> 5), s2, n2b >> 5, full);
-      }
+      if (n2b > 0) bulk_g2s(st + n1b, w2, n2b, full);
       bulk_g2s(st + Cfg::kWBytes, aq, Cfg::kABytes, full);
-      if constexpr (!CH) bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes, sq, Cfg::kSABytes, full);
+      if constexpr (!CH) {
+#pragma unroll
+        for (int gs = 0; gs < GS; ++gs) {               // 2 bytes per row and group
+          const uint32_t dsw = st + Cfg::kWBytes + Cfg::kABytes + gs * (RBB * 16);
+          bulk_g2s(dsw, s1 + gs * kTileRows, n1b >> 5, full);
+          if (n2b > 0) bulk_g2s(dsw + (n1b >> 5), s2 + gs * kTileRows, n2b >> 5, full);
+          bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes + gs * (MT * 32), sq + gs * kTileRows, MT * 32, full);
+        }
+      }
     }
     w1 += kBlobBytes; w2 += kBlobBytes; aq += kBlobBytes;
-    s1 += kTileRows; s2 += kTileRows; sq += kTileRows;
+    s1 += GS * kTileRows; s2 += GS * kTileRows; sq += GS * kTileRows;
     islot = islot + 1 == kStages ? 0 : islot + 1;
     if (++ij == nkw) {
       ij = 0;
@@ -205,11 +214,27 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       // ---- token fragments of this k-block (widened once, reused by every row block)
       uint32_t af[MT][4][4];
       float sa[MT][2];
+      float sag[GS > 1 ? MT : 1][GS][2];                // GS > 1: token scales per group of the k-block
 #pragma unroll
       for (int mi = 0; mi < MT; ++mi) {
         uint32_t x0[4], x1[4];
+        if constexpr (GS > 1) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {                 // word t of chunk c (stored at slot c ^ swizzle)
+            const uint32_t off = q * kRowBytes + ((c ^ ((q >> 1) & 3)) << 4) + 4 * t;
+            x0[c] = lds32(st + Cfg::kWBytes + (16 * mi) * kRowBytes + off);
+            x1[c] = lds32(st + Cfg::kWBytes + (16 * mi + 8) * kRowBytes + off);
+          }
+          const __half* sah = reinterpret_cast<const __half*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes);
+#pragma unroll
+          for (int gs = 0; gs < GS; ++gs) {
+            sag[mi][gs][0] = __half2float(sah[gs * (16 * MT) + 16 * mi + q]);
+            sag[mi][gs][1] = __half2float(sah[gs * (16 * MT) + 16 * mi + q + 8]);
+          }
+        } else {
         lds128(st + Cfg::kWBytes + (16 * mi) * kRowBytes + lane_off, x0[0], x0[1], x0[2], x0[3]);
         lds128(st + Cfg::kWBytes + (16 * mi + 8) * kRowBytes + lane_off, x1[0], x1[1], x1[2], x1[3]);
+        }
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           const uint32_t l0 = rotl4(x0[i]) & kMask, h0 = x0[i] & kMask;
@@ -217,7 +242,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
           af[mi][i][0] = swap ? h0 : l0; af[mi][i][2] = swap ? l0 : h0;   // token q: k lo / hi half
           af[mi][i][1] = swap ? h1 : l1; af[mi][i][3] = swap ? l1 : h1;   // token q + 8
         }
-        if constexpr (!CH) {
+        if constexpr (!CH && GS == 1) {
           const __half* sah = reinterpret_cast<const __half*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes);
           sa[mi][0] = __half2float(sah[16 * mi + q]);
           sa[mi][1] = __half2float(sah[16 * mi + q + 8]);
@@ -228,6 +253,47 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       for (int i = 0; i < RBB; ++i) {
         if (i < nb) {
           uint32_t x[4];
+          if constexpr (GS > 1) {
+            const uint32_t off = q * kRowBytes + 4 * t;
+            const uint32_t swz = (q >> 1) & 3;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) x[c] = lds32(st + i * 512 + off + ((c ^ swz) << 4));
+            constexpr int MPG = 4 / GS;                   // MMAs per group
+#pragma unroll
+            for (int gs = 0; gs < GS; ++gs) {
+              int acc[MT][4];
+#pragma unroll
+              for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) acc[mi][e] = 0;
+#pragma unroll
+              for (int c = gs * MPG; c < (gs + 1) * MPG; ++c) {
+                const uint32_t b0w = rotl4(x[c]) & kMask, b1w = x[c] & kMask;
+#pragma unroll
+                for (int mi = 0; mi < MT; ++mi) mma_s8(acc[mi], af[mi][c], b0w, b1w);
+              }
+              const __half2 sw2 = *reinterpret_cast<const __half2*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + gs * (RBB * 16) + i * 16 + 4 * t);
+              const float sw0 = __low2float(sw2) * 0.00390625f, sw1 = __high2float(sw2) * 0.00390625f;
+#pragma unroll
+              for (int mi = 0; mi < MT; ++mi) {
+                yf[i][mi][0] = fmaf(__int2float_rn(acc[mi][0]) * sw0, sag[mi][gs][0], yf[i][mi][0]);
+                yf[i][mi][1] = fmaf(__int2float_rn(acc[mi][1]) * sw1, sag[mi][gs][0], yf[i][mi][1]);
+                yf[i][mi][2] = fmaf(__int2float_rn(acc[mi][2]) * sw0, sag[mi][gs][1], yf[i][mi][2]);
+                yf[i][mi][3] = fmaf(__int2float_rn(acc[mi][3]) * sw1, sag[mi][gs][1], yf[i][mi][3]);
+                if constexpr (DUMP) {
+                  const int gmm = (kbw0 + j) * GS + gs;
+#pragma unroll
+                  for (int e = 0; e < 4; ++e) {
+                    const int m = 16 * mi + q + 8 * (e >> 1), n = (b0 + i) * 8 + 2 * t + (e & 1);
+                    if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1)
+                      atomicAdd(p.P_out + (static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gmm,
+                                acc[mi][e] >> 8);
+                  }
+                }
+              }
+            }
+            continue;
+          }
           lds128(st + i * 512 + lane_off, x[0], x[1], x[2], x[3]);
           if constexpr (CH) {
 #pragma unroll
@@ -341,20 +407,27 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <int MT, bool CH>
+template <int MT, bool CH, int GS>
 static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaStream_t st) {
-  constexpr int smem = GemvCfg<MT>::kSmemBytes;
+  constexpr int smem = GemvCfg<MT, GS>::kSmemBytes;
   cudaError_t e;
   if (dump) {
-    auto kern = w4a4_gemv_kernel<MT, true, CH>;
+    auto kern = w4a4_gemv_kernel<MT, true, CH, GS>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     kern<<<grid, kThreads, smem, st>>>(p);
   } else {
-    auto kern = w4a4_gemv_kernel<MT, false, CH>;
+    auto kern = w4a4_gemv_kernel<MT, false, CH, GS>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     kern<<<grid, kThreads, smem, st>>>(p);
   }
   return cudaGetLastError();
+}
+template <int MT>
+static cudaError_t launch_gemv_g(const GemmParams& p, bool ch, int gs, bool dump, int grid, cudaStream_t st) {
+  if (ch) return launch_gemv_m<MT, true, 1>(p, dump, grid, st);
+  if (gs == 4) return launch_gemv_m<MT, false, 4>(p, dump, grid, st);
+  if (gs == 2) return launch_gemv_m<MT, false, 2>(p, dump, grid, st);
+  return launch_gemv_m<MT, false, 1>(p, dump, grid, st);
 }
 
 // mt: m16 token tiles (1 or 2; apex4_gemv_ring.cu takes 3 and 4)
@@ -362,9 +435,11 @@ cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaSt
   // one group per k-block (g = 128), or one group for all of K (per-channel, exact INT32 reduction)
   const bool ch = p.G == 1 && p.K > kBlockK;
   if (!ch && p.kbu != 1) return cudaErrorInvalidValue;
+  const int gs = p.g < kBlockK ? kBlockK / p.g : 1;     // groups per k-block (g = 64: 2, g = 32: 4)
+  if (gs != 1 && gs != 2 && gs != 4) return cudaErrorInvalidValue;
   switch (mt) {
-    case 1: return ch ? launch_gemv_m<1, true>(p, dump, grid, st) : launch_gemv_m<1, false>(p, dump, grid, st);
-    case 2: return ch ? launch_gemv_m<2, true>(p, dump, grid, st) : launch_gemv_m<2, false>(p, dump, grid, st);
+    case 1: return launch_gemv_g<1>(p, ch, gs, dump, grid, st);
+    case 2: return launch_gemv_g<2>(p, ch, gs, dump, grid, st);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -187,6 +187,17 @@ def test_gemm_decode_per_channel(A, M, N, K, grid):
     run_gemm_case(A, M, N, K, K, seed=700 + M, dispatch=(0, -1, grid), out_f32=True, sums=None)
 
 
+@pytest.mark.parametrize("M,N,K,g", [(1, 8, 256, 32), (16, 136, 1024, 32), (17, 1000, 512, 64), (32, 8192, 256, 32),
+                                     (20, 264, 2048, 64), (9, 4096, 11008, 32), (5, 64, 28672, 64)])
+@pytest.mark.parametrize("grid", [-1, 3])
+def test_gemm_decode_fine_groups(A, M, N, K, g, grid):
+    """Decode at g = 32 / 64 (M <= 32): every MMA (pair of MMAs) of the decode kernel covers exactly one
+    group and is scaled on its own; group sums bit-exact, outputs inside the tolerance, FP16 and FP32."""
+    assert A.debug_get_dispatch(M, N, K, g)[0] == 0
+    run_gemm_case(A, M, N, K, g, seed=800 + M, dispatch=(0, -1, grid))
+    run_gemm_case(A, M, N, K, g, seed=800 + M, dispatch=(0, -1, grid), out_f32=True, sums=None)
+
+
 @pytest.mark.parametrize("M,N,K,g", [(40, 264, 512, 128), (64, 520, 1024, 32), (100, 520, 1024, 128),
                                      (130, 304, 1024, 512), (300, 520, 1024, 1024), (200, 264, 2048, 64)])
 @pytest.mark.parametrize("dispatch", [(256 + 64, 0, -1), (256 + 128, 0, -1), (256 + 192, 0, -1),
