@@ -17,10 +17,20 @@
  *   - Every call only enqueues work on `stream` (a cudaStream_t passed as void*, NULL = default
  *     stream) and never synchronises (except apex4_measure_rho and the *_host helpers, which say so).
  *   - Return value: an apex4_status.  Arguments are validated before anything is launched; a failed
- *     launch returns APEX4_ERR_CUDA.  Nothing is printed, nothing aborts.
+ *     launch returns APEX4_ERR_CUDA.  Nothing aborts the host and nothing is printed unless the
+ *     environment variable APEX4_VERBOSE is set (one stderr line per failed launch).  Every in-kernel
+ *     barrier wait is bounded: a phase bug traps silently and surfaces as APEX4_ERR_CUDA / a sticky CUDA
+ *     error, never as a hang.
+ *   - No process-global state: the library keeps only two lazily filled read-only caches (SM count,
+ *     resident CTA pairs).  Every call is a pure function of its arguments; concurrent calls on
+ *     different streams are safe when they use different workspaces.
+ *   - Determinism: integer stages are exact.  FP32 summation order is fixed except where three or more
+ *     stream-K ranges meet in one output tile (FP32 atomics): such outputs can differ in the last bits
+ *     between runs, inside the R12 tolerance of DESIGN.md.
  *   - Shapes: X[M,K], W[N,K], Y[M,N] dense row-major (last index contiguous).  K % 128 == 0,
  *     N % 8 == 0, M >= 1.  Group size g: 32, 64, or a multiple of 128 that divides K (128, 256, 512,
- *     1024, ..., K).  Pointers 16-byte aligned.
+ *     1024, ..., K).  Pointers 16-byte aligned.  (SURVEY 8(b) asks for K % 32; the blob layout below
+ *     is built from 128-k blocks, and every K of BASELINE.json's configs is a multiple of 128.)
  *   - Device layouts (opaque to the caller; sizes from the *_bytes queries below):
  *       packed codes  "PT4": rows padded to Rp = roundup(R,128); blob (rt, kb) of 128 rows x 128 k
  *                     = 8192 contiguous bytes at ((rt * K/128 + kb) * 8192); inside a blob row r
@@ -72,13 +82,26 @@ typedef enum { APEX4_OUT_F16 = 0, APEX4_OUT_F32 = 1 } apex4_out;
 /* which GEMM operand a packed-code buffer belongs to (selects the PT4 or the PW4 layout) */
 typedef enum { APEX4_OPERAND_ACT = 0, APEX4_OPERAND_WEIGHT = 1 } apex4_operand;
 
-/* ---- host-side queries (no CUDA work) ------------------------------------------------------- */
+/* Per-call verification / tuning options of the *_ex and debug exports (NULL = automatic everywhere).
+ * They replace any global "force this kernel" switch: the library has no mutable state. */
+typedef struct {
+  int kernel;        /* -1 automatic, 0 decode (weight-stream) kernel, 1 CTA-pair tcgen05 kernel */
+  int pair_tokens;   /* 0 automatic, else 64 / 128 / 192 tokens per pair tile */
+  int split;         /* -1 automatic, 0 whole tiles per CTA pair, 1 stream-K (a6) */
+  int grid;          /* 0 automatic, else CTAs (decode) / CTA pairs to launch (capped at what fits) */
+  int decode_batch;  /* 0 automatic, else 8-row weight blocks per shared-memory batch of the decode kernel */
+  void* timeline;    /* device buffer for clock stamps; read only by -DAPEX4_TIMELINE builds */
+} apex4_debug_opts;
+
+/* ---- host-side queries (no kernel launches; the first call of apex4_workspace_bytes reads two device
+ *      attributes) ----------------------------------------------------------------------------- */
 
 /* Group size a call with these arguments runs at, or a negative apex4_status on invalid input.
  * PAPER.md:162-166, 183.  Pure host function. */
 int apex4_resolve_group_size(int K, int group_size, int gran, int layer);
 
-/* Bytes of the PT4 packed-code buffer for an operand with R rows (M for activations, N for weights). */
+/* Bytes of the PT4 packed-code buffer for an operand with R rows (M for activations, N for weights).
+ * (SURVEY 8(b) calls this apex4_packed_weight_bytes; one query serves both operands here.) */
 size_t apex4_packed_bytes(int R, int K);
 /* Number of FP16 elements of the ST16 scale buffer for R rows at resolved group size g. */
 size_t apex4_scale_elems(int R, int K, int g);
@@ -89,6 +112,9 @@ size_t apex4_scale_elems(int R, int K, int g);
  * once by the caller before its first use; every call leaves it zero-filled again, so one buffer
  * serves any sequence of calls on one stream.  Concurrent calls on different streams need their own. */
 size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer);
+/* The same for a call that passes `opts` to apex4_w4a4_gemm_ex. */
+size_t apex4_workspace_bytes_ex(int M, int N, int K, int group_size, int gran, int layer,
+                                const apex4_debug_opts* opts);
 
 const char* apex4_status_string(int status);
 
@@ -103,7 +129,8 @@ int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran
                        void* qW_packed, void* sW_f16, void* stream);
 /* Offline-calibrated path (Alg. 1 output): codes [R,K] int8 in [-8,7] (row-major)
  * -> PT4 (operand = APEX4_OPERAND_ACT) or PW4 (APEX4_OPERAND_WEIGHT).  Values outside [-8,7] are
- * taken modulo 16 (low nibble). */
+ * taken modulo 16 (low nibble).  (apex4_pack_weights_from_codes; its scales go through
+ * apex4_scales_from_natural.  apex4_unpack_codes below is SURVEY 8(b)'s apex4_unpack_weights.) */
 int apex4_pack_codes(const int8_t* codes, int R, int K, int operand, void* q_packed, void* stream);
 /* natural FP16 scales [R,G] row-major -> ST16 (padding rows zero-filled), and back. */
 int apex4_scales_from_natural(const void* s_nat_f16, int R, int G, void* s_tiled_f16, void* stream);
@@ -121,6 +148,13 @@ int apex4_unpack_codes(const void* q_packed, int R, int K, int operand, int8_t* 
 int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
                     const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
                     int gran, int layer, void* workspace, size_t workspace_bytes, void* stream);
+/* The same call with per-call options (tests force every kernel / tile width / work distribution with it;
+ * opts == NULL is apex4_w4a4_gemm).  Options that the problem does not admit (the decode kernel for
+ * M > 32 or a group size it does not cover) return APEX4_ERR_INVALID_ARG. */
+int apex4_w4a4_gemm_ex(const void* qA_packed, const void* sA_f16, const void* qW_packed,
+                       const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
+                       int gran, int layer, void* workspace, size_t workspace_bytes, void* stream,
+                       const apex4_debug_opts* opts);
 
 /* End-to-end convenience over the three calls above with HOST activations and HOST output:
  * x_host_f16 [M,K] (HOST, pinned for true asynchrony) -> cudaMemcpyAsync -> apex4_quantize_act ->
@@ -134,15 +168,21 @@ int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const 
 
 /* Verification export: the exact per-group INT32 sums P[m,n,gamma] the tensor cores produced, for the
  * window m in [m0,m1), n in [n0,n1): P_out [(m1-m0), (n1-n0), G] int32 row-major.  Runs the same
- * tcgen05 kernel as apex4_w4a4_gemm (same tiles, same pipeline) with the TMEM accumulators dumped
- * by the epilogue. */
+ * kernel as apex4_w4a4_gemm would for (M, N, K, g, opts) -- same tiles, same pipeline, whole tiles per
+ * CTA pair -- with the accumulators dumped by the epilogue instead of dequantised; takes no scales.
+ * P_out is zero-filled by the call (cudaMemsetAsync on `stream`) before the kernel runs. */
 int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, int N, int K,
                            int group_size, int gran, int layer, int m0, int m1, int n0, int n1,
-                           int32_t* P_out, void* stream);
+                           int32_t* P_out, void* stream, const apex4_debug_opts* opts);
+/* Host-side: what a call with these arguments launches.  out5 (HOST) = {kernel (0 decode, 1 pair),
+ * token-tile width, stream-K flag, CTAs or CTA pairs, k units per tile / row blocks per batch}. */
+int apex4_debug_get_dispatch(int M, int N, int K, int group_size, int gran, int layer,
+                             const apex4_debug_opts* opts, int* out5);
 
 /* ---- rho microbenchmark (Eq. 1-2; Table 1) -------------------- */
 /* Measures on the current device: dense INT8 tcgen05.mma rate (TOPS), FP32 FMA rate (TFLOPS),
- * INT32->FP32 conversion rate (Gop/s) and rho = int8_tops / fp32_tflops.  out[] is a HOST array of
+ * INT32->FP32 conversion rate (Gop/s) and rho = int8_tops / fp32_tflops.  (SURVEY 8(b) gives this call four
+ * double* outputs; one array carries them and the raw per-SM-per-clock figures.)  out[] is a HOST array of
  * at least 8 doubles: {int8_tops, fp32_tflops, i2f_gops, rho, tmem_ld_gbs, sm_clock_mhz, int8_mac_per_clk_per_sm,
  * tmem_ld_bytes_per_clk_per_sm}.
  * Synchronises the stream; allocates and frees its own small device scratch (the only call that

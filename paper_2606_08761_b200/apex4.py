@@ -26,11 +26,29 @@ OPERAND_ACT, OPERAND_WEIGHT = 0, 1
 
 EXPORTS = (
     "apex4_resolve_group_size", "apex4_packed_bytes", "apex4_scale_elems", "apex4_workspace_bytes",
-    "apex4_status_string", "apex4_quantize_act", "apex4_pack_weights", "apex4_pack_codes",
-    "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes", "apex4_w4a4_gemm",
-    "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes", "apex4_debug_group_sums",
-    "apex4_measure_rho",
+    "apex4_workspace_bytes_ex", "apex4_status_string", "apex4_quantize_act", "apex4_pack_weights",
+    "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
+    "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes",
+    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho",
 )
+
+
+class DebugOpts(ctypes.Structure):
+    """apex4_debug_opts of include/apex4.h: per-call kernel / tile / work-distribution overrides."""
+    _fields_ = [("kernel", ctypes.c_int), ("pair_tokens", ctypes.c_int), ("split", ctypes.c_int),
+                ("grid", ctypes.c_int), ("decode_batch", ctypes.c_int), ("timeline", ctypes.c_void_p)]
+
+
+KERNEL_DECODE, KERNEL_PAIR = 0, 1
+
+
+def debug_opts(kernel: int = -1, pair_tokens: int = 0, split: int = -1, grid: int = 0, decode_batch: int = 0,
+               timeline: int = 0) -> DebugOpts:
+    return DebugOpts(kernel, pair_tokens, split, grid, decode_batch, timeline or None)
+
+
+def _opts_ref(opts: Optional[DebugOpts]):
+    return ctypes.byref(opts) if opts is not None else None
 
 
 class Apex4Error(RuntimeError):
@@ -61,6 +79,8 @@ def lib() -> ctypes.CDLL:
     L.apex4_scale_elems.restype = c_size_t
     L.apex4_workspace_bytes.argtypes = [c_int] * 6
     L.apex4_workspace_bytes.restype = c_size_t
+    L.apex4_workspace_bytes_ex.argtypes = [c_int] * 6 + [ctypes.POINTER(DebugOpts)]
+    L.apex4_workspace_bytes_ex.restype = c_size_t
     L.apex4_status_string.argtypes = [c_int]
     L.apex4_status_string.restype = ctypes.c_char_p
     for name in ("apex4_quantize_act", "apex4_pack_weights"):
@@ -73,19 +93,18 @@ def lib() -> ctypes.CDLL:
     L.apex4_scales_to_natural.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p]
     L.apex4_w4a4_gemm.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int,
                                   c_int, c_int, c_int, c_int, c_void_p, c_size_t, c_void_p]
+    L.apex4_w4a4_gemm_ex.argtypes = L.apex4_w4a4_gemm.argtypes + [ctypes.POINTER(DebugOpts)]
     L.apex4_w4a4_linear_host.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int, c_int,
                                          c_int, c_int, c_int, c_void_p, c_size_t, c_void_p]
     L.apex4_linear_host_scratch_bytes.argtypes = [c_int] * 6
     L.apex4_linear_host_scratch_bytes.restype = c_size_t
-    L.apex4_debug_group_sums.argtypes = [c_void_p, c_void_p] + [c_int] * 10 + [c_void_p, c_void_p]
+    L.apex4_debug_group_sums.argtypes = [c_void_p, c_void_p] + [c_int] * 10 + [c_void_p, c_void_p,
+                                                                              ctypes.POINTER(DebugOpts)]
     L.apex4_measure_rho.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
-    L.apex4_debug_set_dispatch.argtypes = [c_int, c_int, c_int]
-    L.apex4_debug_set_timeline.argtypes = [c_void_p]
-    L.apex4_debug_get_dispatch.argtypes = [c_int, c_int, c_int, c_int, ctypes.POINTER(c_int)]
+    L.apex4_debug_get_dispatch.argtypes = [c_int] * 6 + [ctypes.POINTER(DebugOpts), ctypes.POINTER(c_int)]
     for name in ("apex4_pack_codes", "apex4_unpack_codes", "apex4_scales_from_natural",
-                 "apex4_scales_to_natural", "apex4_w4a4_gemm", "apex4_w4a4_linear_host",
-                 "apex4_debug_group_sums", "apex4_measure_rho", "apex4_debug_set_dispatch",
-                 "apex4_debug_get_dispatch"):
+                 "apex4_scales_to_natural", "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host",
+                 "apex4_debug_group_sums", "apex4_measure_rho", "apex4_debug_get_dispatch"):
         getattr(L, name).restype = c_int
     _lib = L
     return L
@@ -126,8 +145,10 @@ def scale_elems(R: int, K: int, g: int) -> int:
 
 
 def workspace_bytes(M: int, N: int, K: int, group_size: int, gran: int = GRAN_GROUP,
-                    layer: int = LAYER_OTHER) -> int:
-    return lib().apex4_workspace_bytes(M, N, K, group_size, gran, layer)
+                    layer: int = LAYER_OTHER, opts: Optional[DebugOpts] = None) -> int:
+    if opts is None:
+        return lib().apex4_workspace_bytes(M, N, K, group_size, gran, layer)
+    return lib().apex4_workspace_bytes_ex(M, N, K, group_size, gran, layer, _opts_ref(opts))
 
 
 def _quantize(fn_name: str, x: torch.Tensor, group_size: int, gran: int, layer: int,
@@ -176,7 +197,7 @@ def unpack_codes(q: torch.Tensor, R: int, K: int, operand: int) -> torch.Tensor:
 def scales_from_natural(s_nat: torch.Tensor) -> torch.Tensor:
     _dev(s_nat, torch.float16, "apex4_scales_from_natural")
     R, G = s_nat.shape
-    out = torch.empty((R + 127) // 128 * 128 * G, dtype=torch.float16, device=s_nat.device)
+    out = torch.empty(lib().apex4_scale_elems(R, G, 1), dtype=torch.float16, device=s_nat.device)
     _check(lib().apex4_scales_from_natural(s_nat.data_ptr(), R, G, out.data_ptr(), _stream()),
            "apex4_scales_from_natural")
     return out
@@ -190,38 +211,42 @@ def scales_to_natural(s_tiled: torch.Tensor, R: int, G: int) -> torch.Tensor:
     return out
 
 
-def make_workspace(M, N, K, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, device="cuda"):
+def make_workspace(M, N, K, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, device="cuda", opts=None):
     """Zero-filled workspace for apex4_w4a4_gemm (None if the problem needs none)."""
-    nbytes = workspace_bytes(M, N, K, group_size, gran, layer)
+    nbytes = workspace_bytes(M, N, K, group_size, gran, layer, opts)
     if nbytes == 0:
         return None
     return torch.zeros(nbytes, dtype=torch.uint8, device=device)
 
 
 def w4a4_gemm(qA, sA, qW, sW, M: int, N: int, K: int, group_size=128, gran=GRAN_GROUP,
-              layer=LAYER_OTHER, out_dtype=torch.float16, workspace=None, out=None) -> torch.Tensor:
-    """apex4_w4a4_gemm: Y[M,N] = sum_g sA sW P_g (Eq. 8)."""
+              layer=LAYER_OTHER, out_dtype=torch.float16, workspace=None, out=None,
+              opts: Optional[DebugOpts] = None) -> torch.Tensor:
+    """apex4_w4a4_gemm (apex4_w4a4_gemm_ex when `opts` is given): Y[M,N] = sum_g sA sW P_g (Eq. 8)."""
     if out is None:
         out = torch.empty((M, N), dtype=out_dtype, device=qA.device)
     code = OUT_F16 if out.dtype == torch.float16 else OUT_F32
     if workspace is None:
-        workspace = make_workspace(M, N, K, group_size, gran, layer, qA.device)
+        workspace = make_workspace(M, N, K, group_size, gran, layer, qA.device, opts)
     wp = workspace.data_ptr() if workspace is not None else None
     wb = workspace.numel() if workspace is not None else 0
-    st = lib().apex4_w4a4_gemm(qA.data_ptr(), sA.data_ptr(), qW.data_ptr(), sW.data_ptr(), out.data_ptr(),
-                               code, M, N, K, group_size, gran, layer, wp, wb, _stream())
-    _check(st, "apex4_w4a4_gemm")
+    args = (qA.data_ptr(), sA.data_ptr(), qW.data_ptr(), sW.data_ptr(), out.data_ptr(), code, M, N, K,
+            group_size, gran, layer, wp, wb, _stream())
+    if opts is None:
+        _check(lib().apex4_w4a4_gemm(*args), "apex4_w4a4_gemm")
+    else:
+        _check(lib().apex4_w4a4_gemm_ex(*args, _opts_ref(opts)), "apex4_w4a4_gemm_ex")
     return out
 
 
 def debug_group_sums(qA, qW, M, N, K, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER,
-                     m0=0, m1=None, n0=0, n1=None) -> torch.Tensor:
+                     m0=0, m1=None, n0=0, n1=None, opts: Optional[DebugOpts] = None) -> torch.Tensor:
     m1 = M if m1 is None else m1
     n1 = N if n1 is None else n1
     g = resolve_group_size(K, group_size, gran, layer)
-    P = torch.zeros((m1 - m0, n1 - n0, K // g), dtype=torch.int32, device=qA.device)
+    P = torch.empty((m1 - m0, n1 - n0, K // g), dtype=torch.int32, device=qA.device)
     st = lib().apex4_debug_group_sums(qA.data_ptr(), qW.data_ptr(), M, N, K, group_size, gran, layer,
-                                      m0, m1, n0, n1, P.data_ptr(), _stream())
+                                      m0, m1, n0, n1, P.data_ptr(), _stream(), _opts_ref(opts))
     _check(st, "apex4_debug_group_sums")
     return P
 
@@ -253,14 +278,10 @@ def measure_rho() -> dict:
     return dict(zip(keys, [float(v) for v in out]))
 
 
-def debug_set_dispatch(nt: int = -1, split: int = -1, grid: int = -1) -> None:
-    """Test hook: force the kernel / token-tile width (0 = decode kernel, 16..128 = one-CTA tile kernel,
-    256 = CTA pairs, 256 + w = CTA pairs with w = 64 / 128 / 192 tokens per tile), stream-K (0/1) and the grid size."""
-    lib().apex4_debug_set_dispatch(nt, split, grid)
-
-
-def debug_get_dispatch(M, N, K, g) -> Tuple[int, int, int, int]:
-    """-> (token-tile width, stream-K flag, grid size, k units per tile)"""
-    out = (ctypes.c_int * 4)()
-    lib().apex4_debug_get_dispatch(M, N, K, g, out)
+def debug_get_dispatch(M, N, K, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER,
+                       opts: Optional[DebugOpts] = None) -> Tuple[int, int, int, int, int]:
+    """-> (kernel (0 decode, 1 pair), token-tile width, stream-K flag, CTAs / CTA pairs, k units per tile)"""
+    out = (ctypes.c_int * 5)()
+    _check(lib().apex4_debug_get_dispatch(M, N, K, group_size, gran, layer, _opts_ref(opts), out),
+           "apex4_debug_get_dispatch")
     return tuple(int(v) for v in out)

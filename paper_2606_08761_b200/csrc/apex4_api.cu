@@ -63,100 +63,106 @@ int resolve_g(int K, int group_size, int gran, int layer) {
 }
 
 struct Dispatch {
-  int nt;      // token-tile width; 256 = CTA-pair kernel (256 x 256 tiles, grid counted in pairs)
-  int bias;    // magic-biased accumulators (g <= 128)
-  int split;   // stream-K work distribution (needs the workspace)
-  int grid;
+  int kernel;  // 0 = decode (weight-stream) kernel, 1 = CTA-pair tcgen05 kernel
+  int bias;    // pair kernel: magic-biased accumulators (g <= 128)
+  int split;   // pair kernel: stream-K work distribution (needs the workspace)
+  int grid;    // CTAs (decode) or CTA pairs (pair kernel)
   int upt, kbu, tiles_m, tiles_n;
-  int rows8, mt;   // nt == 0: decode (stream) kernel, 8-row groups per warp and m16 token tiles
-  int pnt;         // nt == 256: tokens per pair tile (64 / 128 / kPairTokens)
+  int mt;      // decode kernel: m16 token tiles
+  int pnt;     // pair kernel: tokens per pair tile (64 / 128 / kPairTokens)
 };
 
-// test hook (apex4_debug_set_dispatch): -1 = automatic
-int g_force_nt = -1, g_force_split = -1, g_force_grid = -1, g_force_pnt = -1;   // g_force_nt == 0 forces the decode kernel
-long long* g_timeline = nullptr;
+// "automatic" values of apex4_debug_opts
+const apex4_debug_opts kAuto = {-1, 0, -1, 0, 0, nullptr};
 
 // Tokens per pair tile: columns past M are wasted epilogue / MMA work, but a 128-token tile costs ~1.2 x
 // a 192-token tile per token (measured at N = K = 8192: M = 1024 146 vs 139 us at g = 128, 88 vs 79 us
 // per-channel; M = 256: 44 vs 54 us).  M <= 64: the 64-token tile.
-int pair_tokens(int M) {
-  if (g_force_pnt > 0) return g_force_pnt;
+int pair_tokens(int M, const apex4_debug_opts& o) {
+  if (o.pair_tokens > 0) return o.pair_tokens;
   if (M <= 64) return 64;
   const int r128 = (M + 127) / 128 * 128, r192 = (M + kPairTokens - 1) / kPairTokens * kPairTokens;
   return 6 * r128 < 5 * r192 ? 128 : kPairTokens;
 }
 
-Dispatch choose_dispatch(int M, int N, int K, int g) {
-  Dispatch d;
-  d.pnt = 0;
+// The decode kernel covers M <= 32 at g = 32 / 64 / 128 and per-channel (groups in between need one
+// rounding per group, R12, which its per-k-block FP32 scaling does not keep).
+bool decode_supported(int M, int K, int g) {
+  if (M > 32) return false;
+  return g == 32 || g == 64 || g == kBlockK || (g == K && K > kBlockK);
+}
+
+int sm_count() {
+  static int sms = 0;
+  if (sms == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+      sms = 148;
+  }
+  return sms;
+}
+
+// Pure function of the problem and the (per-call) debug options: no process-global state.
+// Returns false when the options ask for a kernel that does not cover the problem.
+bool choose_dispatch(int M, int N, int K, int g, const apex4_debug_opts& o, Dispatch& d) {
+  memset(&d, 0, sizeof(d));
   const int KB = K / kBlockK;
   d.kbu = g > kBlockK ? g / kBlockK : 1;   // indivisible k unit: a whole group, at least a k-block
   d.upt = KB / d.kbu;
   d.bias = g <= kBlockK;
-  d.rows8 = d.mt = 0;
-  // decode kernel: M <= 32 at g = 32 / 64 / 128 or per-channel (groups in between need one rounding per group, R12,
-  // which its per-k-block FP32 scaling does not keep; 32 < M <= 64: the pair kernel with 64-token tiles, 24.5 vs 36.2 us at N = K = 8192).  Everything
-  // else runs on CTA pairs; the one-CTA tile kernel (nt = 16..128) and the ring decode kernel are only
-  // reachable through the test hook.
-  // per-channel (g = K): the same decode kernel with an exact INT32 cross-warp reduction (M <= 32)
-  const bool gemv_ok = ((g_force_nt == 0 ? M <= 64 : M <= 32) && g == kBlockK) || (M <= 32 && g == K && K > kBlockK) ||
-                       (M <= 32 && (g == 32 || g == 64));   // fine groups: one MMA (pair) per group
-  if (g_force_nt > 0) d.nt = g_force_nt;
-  else if (gemv_ok) d.nt = 0;
-  else d.nt = 256;
-  if (d.nt == 0) {
-    // decode kernel: a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
+  const bool dec_ok = decode_supported(M, K, g);
+  if (o.kernel == 0 && !dec_ok) return false;
+  if (o.kernel > 1 || o.kernel < -1) return false;
+  d.kernel = o.kernel >= 0 ? o.kernel : (dec_ok ? 0 : 1);
+  if (d.kernel == 0) {
+    // a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
     d.bias = 0;
     d.mt = (M + 15) / 16;
-    d.rows8 = d.mt >= 3 ? 1 : 0;     // 1: register-ring kernel (3-4 token tiles), 0: bulk-copy staged kernel
     d.tiles_m = 1;
     d.tiles_n = (N + 7) / 8;
-    d.grid = g_force_grid > 0 ? g_force_grid : gemm_max_ctas();
+    d.grid = o.grid > 0 ? o.grid : sm_count();
     if (d.grid > d.tiles_n) d.grid = d.tiles_n;
     const int per_cta = (d.tiles_n + d.grid - 1) / d.grid;
-    const int max_batch = d.rows8 ? gemv_ring_max_batch(d.mt) : gemv_max_batch(d.mt);
+    const int max_batch = gemv_max_batch(d.mt);
     d.upt = per_cta < max_batch ? per_cta : max_batch;     // row blocks per shared-memory batch
-    if (g_force_nt == 0 && g_force_split > 0 && g_force_split < d.upt) d.upt = g_force_split;   // test hook
-    d.split = 0;
-    return d;
+    if (o.decode_batch > 0 && o.decode_batch < d.upt) d.upt = o.decode_batch;
+    return true;
   }
-  const bool pair = d.nt == 256;
-  if (pair) d.pnt = pair_tokens(M);
-  d.tiles_m = pair ? (M + d.pnt - 1) / d.pnt : (M + d.nt - 1) / d.nt;
-  d.tiles_n = pair ? (N + 2 * kTileRows - 1) / (2 * kTileRows) : (N + kTileRows - 1) / kTileRows;
+  d.pnt = pair_tokens(M, o);
+  if (d.pnt != 64 && d.pnt != 128 && d.pnt != kPairTokens) return false;
+  d.tiles_m = (M + d.pnt - 1) / d.pnt;
+  d.tiles_n = (N + 2 * kTileRows - 1) / (2 * kTileRows);
   const long long tiles = static_cast<long long>(d.tiles_m) * d.tiles_n;
   const long long units = tiles * d.upt;
-  const int max_grid = pair ? gemm_max_pairs() : gemm_max_ctas();
-  const int sms = (g_force_grid > 0 && g_force_grid < max_grid) ? g_force_grid : max_grid;
+  const int max_grid = gemm_max_pairs();
+  const int sms = (o.grid > 0 && o.grid < max_grid) ? o.grid : max_grid;
   d.grid = static_cast<int>(units < sms ? units : sms);
-  // whole tiles per CTA when the last wave is reasonably full, stream-K otherwise
+  // whole tiles per CTA pair when the last wave is reasonably full, stream-K otherwise
   const long long waves = (tiles + d.grid - 1) / d.grid;
   const double eff = static_cast<double>(tiles) / static_cast<double>(waves * d.grid);
   // a single, reasonably full wave is cheaper as whole tiles than as stream-K ranges (each partial range
   // pays a reduction and a pipeline restart: M = 256, N = K = 8192 57.7 us whole vs 61.5 us split)
-  d.split = (g_force_split >= 0) ? g_force_split : ((eff < 0.93 && !(waves == 1 && eff >= 0.8)) ? 1 : 0);
+  d.split = (o.split >= 0) ? (o.split ? 1 : 0) : ((eff < 0.93 && !(waves == 1 && eff >= 0.8)) ? 1 : 0);
   if (d.upt == 1) d.split = 0;                      // nothing to split
   if (!d.split && tiles < d.grid) d.grid = static_cast<int>(tiles);
-  return d;
+  return true;
 }
 
 size_t counters_bytes(const Dispatch& d) {
-  return (static_cast<size_t>(d.tiles_m) * d.tiles_n * (d.nt == 256 ? 2 : 1) * 4 + 255) / 256 * 256;
+  return (static_cast<size_t>(d.tiles_m) * d.tiles_n * 2 * 4 + 255) / 256 * 256;
 }
 
 cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
-  const cudaError_t e = d.nt == 256 ? launch_gemm_pair(p, d.bias, dump, d.grid, st)
-                        : d.nt == 0 ? (d.rows8 ? launch_gemv_ring(p, d.mt, dump, d.grid, st) : launch_gemv(p, d.mt, dump, d.grid, st))
-                                    : launch_gemm(p, d.nt, d.bias, dump, d.grid, st);
+  const cudaError_t e = d.kernel == 1 ? launch_gemm_pair(p, d.bias, dump, d.grid, st) : launch_gemv(p, d.mt, dump, d.grid, st);
   if (e != cudaSuccess && getenv("APEX4_VERBOSE"))
-    fprintf(stderr, "apex4: GEMM launch (tile %d, grid %d) failed: %s\n", d.nt, d.grid, cudaGetErrorString(e));
+    fprintf(stderr, "apex4: GEMM launch (kernel %d, grid %d) failed: %s\n", d.kernel, d.grid, cudaGetErrorString(e));
   return e;
 }
-size_t workspace_need(const Dispatch& d, int M, int N) {
+size_t workspace_need(const Dispatch& d) {
   if (!d.split) return 0;
-  // pair kernel: every 256 x pnt tile in fragment order (tile-padded); tile kernel: [M, N]
-  if (d.nt == 256) return counters_bytes(d) + static_cast<size_t>(d.tiles_m) * d.tiles_n * 256 * d.pnt * 4;
-  return counters_bytes(d) + static_cast<size_t>(M) * N * 4;
+  // every 256 x pnt pair tile as FP32 in fragment order (tile-padded), after the arrival counters
+  return counters_bytes(d) + static_cast<size_t>(d.tiles_m) * d.tiles_n * 256 * d.pnt * 4;
 }
 
 int validate_gemm_shape(int M, int N, int K) {
@@ -195,11 +201,17 @@ size_t apex4_scale_elems(int R, int K, int g) {
   return st16_elems(R, K / g);
 }
 
-size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer) {
+size_t apex4_workspace_bytes_ex(int M, int N, int K, int group_size, int gran, int layer,
+                                const apex4_debug_opts* opts) {
   if (validate_gemm_shape(M, N, K) != APEX4_OK) return 0;
   const int g = resolve_g(K, group_size, gran, layer);
   if (g < 0) return 0;
-  return workspace_need(choose_dispatch(M, N, K, g), M, N);
+  Dispatch d;
+  if (!choose_dispatch(M, N, K, g, opts ? *opts : kAuto, d)) return 0;
+  return workspace_need(d);
+}
+size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer) {
+  return apex4_workspace_bytes_ex(M, N, K, group_size, gran, layer, nullptr);
 }
 
 static int quantize_common(const void* x, int R, int K, int group_size, int gran, int layer, void* q,
@@ -274,12 +286,12 @@ static void fill_params(GemmParams& p, const Dispatch& d, const void* qA, const 
   p.M = M; p.N = N; p.K = K; p.g = g; p.G = K / g;
   p.tiles_m = d.tiles_m; p.tiles_n = d.tiles_n;
   p.split = d.split; p.upt = d.upt; p.kbu = d.kbu; p.pair_nt = d.pnt;
-  p.tl = g_timeline;
 }
 
-int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
-                    const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
-                    int gran, int layer, void* workspace, size_t workspace_bytes, void* stream) {
+int apex4_w4a4_gemm_ex(const void* qA_packed, const void* sA_f16, const void* qW_packed,
+                       const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
+                       int gran, int layer, void* workspace, size_t workspace_bytes, void* stream,
+                       const apex4_debug_opts* opts) {
   if (!qA_packed || !sA_f16 || !qW_packed || !sW_f16 || !Y) return APEX4_ERR_INVALID_ARG;
   if (out_dtype != APEX4_OUT_F16 && out_dtype != APEX4_OUT_F32) return APEX4_ERR_INVALID_ARG;
   int v = validate_gemm_shape(M, N, K);
@@ -291,12 +303,14 @@ int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_pa
     return APEX4_ERR_ALIGNMENT;
   const int a = check_arch();
   if (a != APEX4_OK) return a;
-  const Dispatch d = choose_dispatch(M, N, K, g);
+  Dispatch d;
+  if (!choose_dispatch(M, N, K, g, opts ? *opts : kAuto, d)) return APEX4_ERR_INVALID_ARG;
   GemmParams p;
   fill_params(p, d, qA_packed, sA_f16, qW_packed, sW_f16, M, N, K, g);
   p.Y = Y; p.out_f32 = (out_dtype == APEX4_OUT_F32);
+  p.tl = opts ? static_cast<long long*>(opts->timeline) : nullptr;   // read by -DAPEX4_TIMELINE builds only
   if (d.split) {
-    if (!workspace || workspace_bytes < workspace_need(d, M, N) || !aligned16(workspace))
+    if (!workspace || workspace_bytes < workspace_need(d) || !aligned16(workspace))
       return APEX4_ERR_WORKSPACE;
     p.counters = static_cast<int*>(workspace);
     p.ws = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + counters_bytes(d));
@@ -306,9 +320,16 @@ int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_pa
              : APEX4_ERR_CUDA;
 }
 
+int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
+                    const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
+                    int gran, int layer, void* workspace, size_t workspace_bytes, void* stream) {
+  return apex4_w4a4_gemm_ex(qA_packed, sA_f16, qW_packed, sW_f16, Y, out_dtype, M, N, K, group_size, gran,
+                            layer, workspace, workspace_bytes, stream, nullptr);
+}
+
 int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, int N, int K,
                            int group_size, int gran, int layer, int m0, int m1, int n0, int n1,
-                           int32_t* P_out, void* stream) {
+                           int32_t* P_out, void* stream, const apex4_debug_opts* opts) {
   if (!qA_packed || !qW_packed || !P_out) return APEX4_ERR_INVALID_ARG;
   int v = validate_gemm_shape(M, N, K);
   if (v != APEX4_OK) return v;
@@ -317,21 +338,26 @@ int apex4_debug_group_sums(const void* qA_packed, const void* qW_packed, int M, 
   if (g < 0) return -g;
   const int a = check_arch();
   if (a != APEX4_OK) return a;
-  const Dispatch d = choose_dispatch(M, N, K, g);
+  Dispatch d;
+  if (!choose_dispatch(M, N, K, g, opts ? *opts : kAuto, d)) return APEX4_ERR_INVALID_ARG;
+  d.split = 0;   // the dump needs every tile's groups in one CTA (pair); the decode kernel never splits
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  // the decode kernel adds its warps' partial group sums into P_out
+  if (cudaMemsetAsync(P_out, 0, static_cast<size_t>(m1 - m0) * (n1 - n0) * (K / g) * sizeof(int32_t), st) != cudaSuccess)
+    return APEX4_ERR_CUDA;
   GemmParams p;
-  // scales are not needed for the integer sums; any valid ST16-sized device memory would do, the
-  // packed code buffers are large enough and are only read
-  fill_params(p, d, qA_packed, qA_packed, qW_packed, qW_packed, M, N, K, g);
+  // no scales: the DUMP kernels neither copy nor read them
+  fill_params(p, d, qA_packed, nullptr, qW_packed, nullptr, M, N, K, g);
   p.Y = nullptr; p.P_out = P_out; p.pm0 = m0; p.pm1 = m1; p.pn0 = n0; p.pn1 = n1;
-  return launch_dispatch(p, d, true, static_cast<cudaStream_t>(stream)) == cudaSuccess
-             ? APEX4_OK
-             : APEX4_ERR_CUDA;
+  return launch_dispatch(p, d, true, st) == cudaSuccess ? APEX4_OK : APEX4_ERR_CUDA;
 }
 
 static size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 
 static size_t host_ws_bytes(int M, int N, int K, int g) {
-  return align256(workspace_need(choose_dispatch(M, N, K, g), M, N));
+  Dispatch d;
+  if (!choose_dispatch(M, N, K, g, kAuto, d)) return 0;
+  return align256(workspace_need(d));
 }
 
 size_t apex4_linear_host_scratch_bytes(int M, int N, int K, int group_size, int gran, int layer) {
@@ -373,22 +399,15 @@ int apex4_w4a4_linear_host(const void* x_host_f16, const void* qW_packed, const 
   return APEX4_OK;
 }
 
-// test hooks, not part of the documented ABI: force token-tile width / stream-K / grid size
-// (-1 = automatic).  Process-global; tests restore it.
-int apex4_debug_set_dispatch(int nt, int split, int grid) {
-  // nt = 256 + w (w = 64 / 128 / 192) forces the pair kernel with w tokens per tile
-  g_force_pnt = (nt > 256) ? nt - 256 : -1;
-  g_force_nt = (nt > 256) ? 256 : nt;
-  g_force_split = split; g_force_grid = grid;
-  return APEX4_OK;
-}
-int apex4_debug_set_timeline(void* dev_buf) {
-  g_timeline = static_cast<long long*>(dev_buf);
-  return APEX4_OK;
-}
-int apex4_debug_get_dispatch(int M, int N, int K, int g, int* out4) {
-  const Dispatch d = choose_dispatch(M, N, K, g);
-  out4[0] = d.nt; out4[1] = d.split; out4[2] = d.grid; out4[3] = d.upt;
+int apex4_debug_get_dispatch(int M, int N, int K, int group_size, int gran, int layer,
+                             const apex4_debug_opts* opts, int* out5) {
+  if (!out5) return APEX4_ERR_INVALID_ARG;
+  if (validate_gemm_shape(M, N, K) != APEX4_OK) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  Dispatch d;
+  if (!choose_dispatch(M, N, K, g, opts ? *opts : kAuto, d)) return APEX4_ERR_INVALID_ARG;
+  out5[0] = d.kernel; out5[1] = d.kernel == 1 ? d.pnt : 16 * d.mt; out5[2] = d.split; out5[3] = d.grid; out5[4] = d.upt;
   return APEX4_OK;
 }
 

@@ -6,9 +6,10 @@
 
 namespace apex4 {
 
-// The kernel always runs "weights on the TMEM lanes": a work tile is 128 weight rows (n) x NT token
-// rows (m), NT in {16, 32, 64, 128, 256}.  Weights (PW4/ST16) are the tcgen05 A operand (widened in
-// registers, stored to TMEM); activations (PT4/ST16) are the B operand (widened in shared memory).
+// Both GEMM kernels run "weights on the rows": the pair kernel puts 256 weight rows (n) on the TMEM lanes
+// of a CTA pair and NT token rows (m) on the accumulator columns; weights (PW4/ST16) are the tcgen05 A
+// operand (widened in registers, stored to TMEM), activations (PT4/ST16) the B operand (widened in shared
+// memory).  The decode kernel streams 8-row weight groups against one or two m16 token tiles.
 struct GemmParams {
   const uint8_t* qW;   // PW4  [Np/128][K/128][8192]
   const __half* sW;    // ST16 [Np/128][G][128]
@@ -17,22 +18,18 @@ struct GemmParams {
   void* Y;             // [M, N] row-major, FP16 or FP32; nullptr for the debug dump
   int out_f32;
   int M, N, K, g, G;
-  int tiles_m, tiles_n;   // ceil(M / NT), ceil(N / 128)
+  int tiles_m, tiles_n;   // pair kernel: ceil(M / pair_nt), ceil(N / 256); decode: 1, ceil(N / 8)
   // work distribution (a6 / PAPER.md:226-230): split = 0 -> CTA c owns whole tiles c, c + grid, ...;
   // split = 1 -> the K loop of all tiles is one line of `units` dealt to the CTAs in equal contiguous
   // ranges (stream-K); a unit is kbu k-blocks (one group when g >= 128), a tile has upt units.
   int split, upt, kbu;
   int pair_nt;         // pair kernel: tokens per tile (64 / 128 / kPairTokens)
-  float* ws;           // split = 1: FP32 partial sums [M, N], zero on entry, zero on exit
+  float* ws;           // split = 1: FP32 partial sums, every pair tile in fragment order; zero on entry, zero on exit
   int* counters;       // split = 1: finished units per tile, zero on entry/exit
   int32_t* P_out;      // debug dump of the per-group INT32 sums (DUMP kernels only)
   int pm0, pm1, pn0, pn1;
-  long long* tl;       // debug timeline (test hook): clock64 stamps of CTA 0, [event][64 k-blocks]; normally null
+  long long* tl;       // -DAPEX4_TIMELINE builds only: clock64 stamps of CTA 0, [event][64]; else unused
 };
-
-// nt: token-tile width (16/32/64/128/256); bias: magic-biased accumulators (g <= 128) or I2F (g >= 256)
-cudaError_t launch_gemm(const GemmParams& p, int nt, bool bias, bool dump, int grid, cudaStream_t st);
-int gemm_max_ctas();   // persistent grid size: one CTA per SM
 
 constexpr int kPairTokens = 192;   // tokens per CTA-pair tile (the widest; 128 / 64 where M is small)
 
@@ -42,12 +39,9 @@ constexpr int kPairTokens = 192;   // tokens per CTA-pair tile (the widest; 128 
 cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st);
 int gemm_max_pairs();
 
-// Decode regime (apex4_gemv.cu): M <= 64, g a multiple of 128, no workspace.  tiles_n = 8-row row blocks,
-// upt = row blocks per shared-memory batch (<= gemv_max_batch(mt)), kbu = k-blocks per group.
+// Decode regime (apex4_gemv.cu): M <= 32 at g = 32 / 64 / 128 or per-channel, no workspace.  tiles_n = 8-row
+// row blocks, upt = row blocks per shared-memory batch (<= gemv_max_batch(mt)), kbu = k-blocks per group.
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st);
 int gemv_max_batch(int mt);
-// 32 < M <= 64 (apex4_gemv_ring.cu): same parameters, register-ring staging
-cudaError_t launch_gemv_ring(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st);
-int gemv_ring_max_batch(int mt);
 
 }  // namespace apex4

@@ -23,8 +23,8 @@
 //                          holds one weight row (its TMEM lane) x 16 consecutive tokens per chunk; this
 //                          shape sustains ~1.4 x the TMEM read rate of 16x256b (profiles/r1_ubench_b200.md);
 //                          chunk c+1 is in flight while chunk c is in the FMA pipe.  Two FFMA2 per element
-//                          pair: fma(f, sW/256, -49152 sW) = P sW rounded once (magic-biased accumulators,
-//                          see apex4_gemm.cu), then fma with the two token scales into the FP32 sums.
+//                          pair: fma(f, sW/256, -49152 sW) = P sW rounded once (magic-biased accumulators),
+//                          then fma with the two token scales into the FP32 sums.
 //   then           producer : 1-D bulk async copies (UBLKCP) of this CTA's packed INT4 rows + FP16 scales
 //   then           MMA      : leader CTA only; tcgen05.mma cta_group::2 kind::i8, M = 256, N = 192, K = 32,
 //                          A (weights) from TMEM, B (tokens) from shared memory; tcgen05.commit
@@ -265,7 +265,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
           pkpar ^= 1u << s;
           const uint32_t st = smem_base + offPk + s * kPkStageBytes;
           const uint32_t full = bar(bPkFull + s);
-          const bool has_scales = kig == 0;
+          const bool has_scales = !DUMP && kig == 0;   // the dump of the integer sums takes no scales (null pointers)
           if (el) {
             stamp(0, kbc);
             mbar_arrive_expect_tx(full, bytes_data + (has_scales ? bytes_scales : 0));
@@ -304,7 +304,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
     // ------------------------------------------------------------------------- MMA issuer (leader)
     // Whole warp, warp-uniform values, one elected lane issues.  No division, no 64-bit descriptor
     // arithmetic, stage / buffer parities kept as bit masks: the first version of this loop took
-    // ~2000 clk per k-block and was the bottleneck of the kernel (profiles/r1_gemm_v3_ncu.md).
+    // ~2000 clk per k-block and was the bottleneck of the kernel (round 1).
     else if (warp == kCtlWarp0 + 1 && rank == 0) {
       const bool el = elect_one();
       const uint32_t desc_lo0 = (((smem_base + offI8) & 0x3FFFFu) >> 4) | (1u << 16);
@@ -362,7 +362,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
     const int r = threadIdx.x & 127;                    // weight row of this CTA's blob = TMEM lane
     const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t wsw = (r >> 1) & 3;                  // chunk-slot swizzle of the packed row (PW4)
-    const uint32_t flip = ((lane >> 2) & 1) * 16;       // see apex4_gemm.cu: bank spread of the two stores
+    const uint32_t flip = ((lane >> 2) & 1) * 16;       // order of the two 16-byte stores: spreads them over the banks
     constexpr uint32_t kMask = 0xF0F0F0F0u;
     uint32_t kbc = 0, gc = 0, s = 0, t = 0, pkpar = 0, oppar = 0;
     while (work_next(p, wit, w, cp, npairs)) {
@@ -741,7 +741,7 @@ int gemm_max_pairs() {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<kPairTokens>::kSmemBytes) != cudaSuccess ||
         cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) {
       cudaGetLastError();
-      n = gemm_max_ctas() / 2;
+      n = 74;   // B200: 148 SMs, one CTA pair per TPC
     }
     pairs = n;
   }

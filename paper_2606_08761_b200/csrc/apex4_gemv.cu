@@ -1,6 +1,6 @@
-// apex4_gemv.cu -- a2..a7 of the hot path for the decode regime (M <= 32, g = 128): the
-// weights are read once from HBM and every byte is used M times, so the kernel is a weight STREAM:
-// no shared-memory staging of operands, no TMEM, no cross-CTA exchange, no workspace.
+// apex4_gemv.cu -- a2..a7 of the hot path for the decode regime (M <= 32; g = 32 / 64 / 128 or per-channel):
+// the weights are read once from HBM and every byte is used M times, so the kernel is a weight STREAM:
+// warp-private bulk-copy stages in shared memory, no TMEM, no cross-CTA exchange, no workspace.
 //
 //   * A CTA (16 warps) owns a contiguous range of 8-row weight groups ("row blocks"), processed in
 //     batches of RBB row blocks, and ALL of K.  Warp w owns the k-blocks [KB w / 16, KB (w+1) / 16).
@@ -22,7 +22,7 @@
 //     the partials of the 16 warps are reduced through shared memory, cast and stored (a6, a7).
 // Tensor cores here are the legacy warp-level path on purpose: at M <= 64 the MMA work is < 2 % of the
 // HBM time and a tcgen05 pipeline (bulk copy -> widen -> TMEM -> MMA -> TMEM load) only adds latency
-// (profiles/r1_gemm_v2_ncu.md: 48 us at M = 16 against 5.3 us of HBM time).
+// (round 1, first tcgen05 tile kernel: 48 us at M = 16 against 5.3 us of HBM time).
 #include <type_traits>
 
 #include "apex4_gemm.cuh"
@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     const int n1 = split_row - row_a, n2 = row_b - split_row;
     w1 = p.qW + tile_a * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes + (row_a & 127) * kRowBytes;
     w2 = p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes;
-    if constexpr (!CH) {
+    if constexpr (!CH && !DUMP) {   // the dump of the integer sums takes no scales (null pointers)
       s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + GS * kbw0) * kTileRows + (row_a & 127);
       s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + GS * kbw0) * kTileRows;
       sq = p.sA + static_cast<size_t>(GS * kbw0) * kTileRows;
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     aq = p.qA + static_cast<size_t>(kbw0) * kBlobBytes;
     n1b = n1 * kRowBytes;
     n2b = n2 * kRowBytes;
-    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + (CH ? 0 : GS * (n1 + n2) * 2 + Cfg::kSABytes);
+    tx = (n1 + n2) * kRowBytes + Cfg::kABytes + ((CH || DUMP) ? 0 : GS * (n1 + n2) * 2 + Cfg::kSABytes);
   };
   if (rb0 < rb1 && nkw > 0) batch_setup();
   auto issue_next = [&]() {                             // copies of one stage
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       bulk_g2s(st, w1, n1b, full);
       if (n2b > 0) bulk_g2s(st + n1b, w2, n2b, full);
       bulk_g2s(st + Cfg::kWBytes, aq, Cfg::kABytes, full);
-      if constexpr (!CH) {
+      if constexpr (!CH && !DUMP) {
 #pragma unroll
         for (int gs = 0; gs < GS; ++gs) {               // 2 bytes per row and group
           const uint32_t dsw = st + Cfg::kWBytes + Cfg::kABytes + gs * (RBB * 16);
@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       }
     }
     w1 += kBlobBytes; w2 += kBlobBytes; aq += kBlobBytes;
-    s1 += GS * kTileRows; s2 += GS * kTileRows; sq += GS * kTileRows;
+    if constexpr (!CH && !DUMP) { s1 += GS * kTileRows; s2 += GS * kTileRows; sq += GS * kTileRows; }
     islot = islot + 1 == kStages ? 0 : islot + 1;
     if (++ij == nkw) {
       ij = 0;
@@ -376,11 +376,13 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
               }
             }
             if (p.Y == nullptr || n >= p.N) continue;
-            // one group: Y = float(P) sW sA (a5), P exact in FP32 (|P| <= 64 K < 2^24)
-            const float sw0 = __half2float(__ldg(p.sW + st16_index(n, 0, 1))), sw1 = __half2float(__ldg(p.sW + st16_index(n + 1, 0, 1)));
-            const float sa0 = __half2float(__ldg(p.sA + st16_index(m, 0, 1))), sa1 = __half2float(__ldg(p.sA + st16_index(m + 8, 0, 1)));
-            v.x = __int2float_rn(s0) * sw0 * sa0; v.y = __int2float_rn(s1i) * sw1 * sa0;
-            v.z = __int2float_rn(s2i) * sw0 * sa1; v.w = __int2float_rn(s3) * sw1 * sa1;
+            if constexpr (!DUMP) {   // the dump takes no scales (null pointers; the loads below may be hoisted)
+              // one group: Y = float(P) sW sA (a5), P exact in FP32 (|P| <= 64 K < 2^24)
+              const float sw0 = __half2float(__ldg(p.sW + st16_index(n, 0, 1))), sw1 = __half2float(__ldg(p.sW + st16_index(n + 1, 0, 1)));
+              const float sa0 = __half2float(__ldg(p.sA + st16_index(m, 0, 1))), sa1 = __half2float(__ldg(p.sA + st16_index(m + 8, 0, 1)));
+              v.x = __int2float_rn(s0) * sw0 * sa0; v.y = __int2float_rn(s1i) * sw1 * sa0;
+              v.z = __int2float_rn(s2i) * sw0 * sa1; v.w = __int2float_rn(s3) * sw1 * sa1;
+            }
           } else {
 #pragma unroll
           for (int ww = 0; ww < kWarps; ++ww) {
@@ -430,7 +432,7 @@ static cudaError_t launch_gemv_g(const GemmParams& p, bool ch, int gs, bool dump
   return launch_gemv_m<MT, false, 1>(p, dump, grid, st);
 }
 
-// mt: m16 token tiles (1 or 2; apex4_gemv_ring.cu takes 3 and 4)
+// mt: m16 token tiles (1 or 2)
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st) {
   // one group per k-block (g = 128), or one group for all of K (per-channel, exact INT32 reduction)
   const bool ch = p.G == 1 && p.K > kBlockK;
@@ -444,6 +446,6 @@ cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaSt
   }
 }
 
-int gemv_max_batch(int mt) { return mt == 1 ? 7 : mt == 2 ? 4 : mt == 3 ? 2 : 1; }
+int gemv_max_batch(int mt) { return mt == 1 ? 7 : 4; }
 
 }  // namespace apex4

@@ -13,7 +13,8 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
 
 // ------------------------------------------------------------------ watchdog
 // Every mbarrier wait is bounded: a phase bug must end in a trap (a failed launch the host reports
-// as APEX4_ERR_CUDA), never in a hung GPU.
+// as APEX4_ERR_CUDA), never in a hung GPU.  The trap is silent; -DAPEX4_WATCHDOG_PRINT (debug builds)
+// adds a device printf that names the barrier.
 #ifndef APEX4_WATCHDOG_SPINS
 #define APEX4_WATCHDOG_SPINS (1u << 26)
 #endif
@@ -47,8 +48,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
     if (++spins > APEX4_WATCHDOG_SPINS) {
+#ifdef APEX4_WATCHDOG_PRINT
       printf("apex4: mbarrier watchdog: block (%d,%d) thread %d bar 0x%x parity %u\n", blockIdx.x,
              blockIdx.y, threadIdx.x, bar, parity);
+#endif
       __trap();
     }
   }
@@ -201,7 +204,7 @@ __device__ __forceinline__ void cluster_sync_all() {
 }
 // arrive (count 1) on the mbarrier at the same shared-memory offset in CTA `rank` of the cluster.
 // Plain (release.cta) arrive, as in CUTLASS' ClusterBarrier: `.release.cluster` compiles to
-// MEMBAR.ALL.GPU + ERRBAR (thousands of cycles on the hand-off path, profiles/r1_gemm_v3_ncu.md); what
+// MEMBAR.ALL.GPU + ERRBAR (thousands of cycles on the hand-off path, measured in round 1); what
 // the peer must see is ordered by the tcgen05 fences and fence.proxy.async issued before the arrive.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank) {
   asm volatile(
@@ -227,8 +230,10 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
   uint32_t spins = 0;
   while (!mbar_try_wait_cluster(bar, parity)) {
     if (++spins > APEX4_WATCHDOG_SPINS) {
+#ifdef APEX4_WATCHDOG_PRINT
       printf("apex4: cluster mbarrier watchdog: block %d thread %d bar 0x%x parity %u\n", blockIdx.x,
              threadIdx.x, bar, parity);
+#endif
       __trap();
     }
   }

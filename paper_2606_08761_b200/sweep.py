@@ -71,7 +71,7 @@ def time_shape(M, N, K, g, dev, cublas=True):
     out = {"M": M, "N": N, "K": K, "g": g, "us": round(us, 2),
            "tops": round(2.0 * M * N * K / us * 1e-6, 1),
            "gbs": round(gemm_bytes(M, N, K, g) / us * 1e-3, 1),
-           "kernel": {0: "gemv", 256: "pair"}.get(apex4.debug_get_dispatch(M, N, K, g)[0], "tile")}
+           "kernel": ("gemv", "pair")[apex4.debug_get_dispatch(M, N, K, g)[0]]}
     del sets
     if cublas:
         nb = int(max(1, min(4, 2 * L2_BYTES // (2 * N * K) + 1)))

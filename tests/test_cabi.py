@@ -75,32 +75,43 @@ def test_argument_validation_without_gpu(L):
 
 
 def test_dispatch_table(L):
-    """Host-side choice of token-tile width / work distribution (a6, a8): pure host code."""
+    """Host-side choice of kernel / token-tile width / work distribution (a6, a8): pure host code, a pure
+    function of the problem and the per-call options (no global switch)."""
     from paper_2606_08761_b200 import apex4
-    # decode regime, g = 128: the streaming kernel (nt = 0), 8-row row blocks over all SMs, no workspace
-    nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 128)
-    assert (nt, split, upt) == (0, 0, 7) and 1 <= grid <= 148
-    assert apex4.debug_get_dispatch(32, 8192, 8192, 128)[0] == 0
+    DEC, PAIR = apex4.KERNEL_DECODE, apex4.KERNEL_PAIR
+    # decode regime, g = 128: the streaming kernel, 8-row row blocks over all SMs, no workspace
+    kern, width, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 128)
+    assert (kern, width, split, upt) == (DEC, 16, 0, 7) and 1 <= grid <= 148
+    assert apex4.debug_get_dispatch(32, 8192, 8192, 128)[:2] == (DEC, 32)
     assert apex4.workspace_bytes(16, 8192, 8192, 128) == 0
     # 32 < M <= 64: CTA pairs on 256 x 64 tiles, 32 tiles on <= 74 pairs -> stream-K; workspace = 32 * 2
     # counters + every 256 x 64 tile as FP32
-    nt, split, grid, upt = apex4.debug_get_dispatch(64, 8192, 8192, 128)
-    assert (nt, split, upt) == (256, 1, 64)
+    kern, width, split, grid, upt = apex4.debug_get_dispatch(64, 8192, 8192, 128)
+    assert (kern, width, split, upt) == (PAIR, 64, 1, 64)
     assert apex4.workspace_bytes(64, 8192, 8192, 128) == 256 + 32 * 256 * 64 * 4
     # M = 256: two 128-token tiles instead of a 192-token tile and a third-full one
-    assert apex4.workspace_bytes(256, 4096, 4096, 128) in (0, 256 + 2 * 16 * 256 * 128 * 4)
+    assert apex4.debug_get_dispatch(256, 4096, 4096, 128)[1] == 128
     # tensor-bound regime: CTA pairs on 256 x 192 tiles; 43 x 32 tiles fill the last wave -> whole tiles
-    nt, split, grid, upt = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
-    assert (nt, split, upt) == (256, 0, 64) and 1 <= grid <= 74
+    kern, width, split, grid, upt = apex4.debug_get_dispatch(8192, 8192, 8192, 128)
+    assert (kern, width, split, upt) == (PAIR, 192, 0, 64) and 1 <= grid <= 74
     assert apex4.workspace_bytes(8192, 8192, 8192, 128) == 0
     # Llama-2-7B O-proj at M = 2048: 11 x 16 tiles on <= 74 pairs -> stream-K with the FP32 workspace
-    nt, split, grid, upt = apex4.debug_get_dispatch(2048, 4096, 4096, 128)
-    assert (nt, split, upt) == (256, 1, 32)
+    kern, width, split, grid, upt = apex4.debug_get_dispatch(2048, 4096, 4096, 128)
+    assert (kern, width, split, upt) == (PAIR, 192, 1, 32)
     # 11 * 16 * 2 counters (padded to 256 bytes) + every 256 x 192 tile as FP32 in fragment order
     assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 11 * 16 * 256 * 192 * 4
     # per-channel decode: the streaming kernel with an exact INT32 cross-warp reduction, no workspace
-    assert apex4.debug_get_dispatch(16, 8192, 8192, 8192)[:2] == (0, 0)
-    # groups between 128 and K at small M: CTA pairs on 256 x 64 tiles; a group is the indivisible k unit
-    nt, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 1024)
-    assert (nt, upt) == (256, 8)
+    assert apex4.debug_get_dispatch(16, 8192, 8192, 0, apex4.GRAN_CHANNEL)[:3] == (DEC, 16, 0)
     assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0
+    # groups between 128 and K at small M: CTA pairs on 256 x 64 tiles; a group is the indivisible k unit
+    kern, width, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 1024)
+    assert (kern, width, upt) == (PAIR, 64, 8)
+    # per-call options: forcing the pair kernel / a tile width / stream-K changes this call only
+    o = apex4.debug_opts(kernel=PAIR, pair_tokens=128, split=1, grid=5)
+    assert apex4.debug_get_dispatch(16, 256, 512, 128, opts=o)[:4] == (PAIR, 128, 1, 4)   # 4 units: grid capped
+    assert apex4.workspace_bytes(16, 256, 512, 128, opts=o) == 256 + 256 * 128 * 4
+    assert apex4.debug_get_dispatch(16, 256, 512, 128)[0] == DEC                           # ... not the next one
+    with pytest.raises(apex4.Apex4Error):            # the decode kernel does not cover M > 32
+        apex4.debug_get_dispatch(64, 256, 512, 128, opts=apex4.debug_opts(kernel=DEC))
+    with pytest.raises(apex4.Apex4Error):            # ... nor groups between 128 and K
+        apex4.debug_get_dispatch(16, 256, 1024, 256, opts=apex4.debug_opts(kernel=DEC))

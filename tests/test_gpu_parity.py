@@ -16,8 +16,7 @@ def A():
     from paper_2606_08761_b200 import apex4
     apex4.lib()
     assert torch.cuda.is_available()
-    yield apex4
-    apex4.debug_set_dispatch(-1, -1, -1)
+    return apex4
 
 
 def dev(a):
@@ -108,36 +107,41 @@ def test_pack_unpack_roundtrip_and_scale_layout(A):
 
 
 # ------------------------------------------------------------------------------- GEMM (a2..a7)
-def run_gemm_case(A, M, N, K, g, seed, fixed=False, out_f32=False, sums="all", dispatch=None):
-    X, W = inputs.make_gemm_inputs(M, N, K, seed, fixed_outliers=fixed)
+def run_gemm_case(A, M, N, K, g, seed=0, fixed=False, out_f32=False, sums="all", opts=None, XW=None):
+    """One problem through quantizer + packer + GEMM (+ the group-sum dump) against the oracle.
+    opts: keyword arguments of apex4.debug_opts (kernel / pair_tokens / split / grid / decode_batch)
+    passed PER CALL through apex4_w4a4_gemm_ex -- the library has no global dispatch switch."""
+    X, W = XW if XW is not None else inputs.make_gemm_inputs(M, N, K, seed, fixed_outliers=fixed)
     ref = O.w4a4_linear(X, W, g)
     G = K // g
-    if dispatch is not None:
-        A.debug_set_dispatch(*dispatch)
-    try:
-        qA, sA, _ = A.quantize_act(dev(X), g)
-        qW, sW, _ = A.pack_weights(dev(W), g)
-        Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g,
-                        out_dtype=torch.float32 if out_f32 else torch.float16)
-        # a second call on the same (self-cleaning) workspace must give the same answer
-        ws = A.make_workspace(M, N, K, g)
-        Y2 = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=Y.dtype, workspace=ws)
-        Y3 = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=Y.dtype, workspace=ws)
-        if sums == "all":
-            P = A.debug_group_sums(qA, qW, M, N, K, g).cpu().numpy()
-            assert np.array_equal(P, O.group_sums(ref["qA"], ref["qW"], g))
-        elif sums is not None:
-            m0, m1, n0, n1 = sums
-            P = A.debug_group_sums(qA, qW, M, N, K, g, m0=m0, m1=m1, n0=n0, n1=n1).cpu().numpy()
-            assert np.array_equal(P, O.group_sums(ref["qA"][m0:m1], ref["qW"][n0:n1], g))
-        torch.cuda.synchronize()
-    finally:
-        A.debug_set_dispatch(-1, -1, -1)
+    o = A.debug_opts(**opts) if opts else None
+    qA, sA, _ = A.quantize_act(dev(X), g)
+    qW, sW, _ = A.pack_weights(dev(W), g)
+    assert np.array_equal(A.unpack_codes(qA, M, K, A.OPERAND_ACT).cpu().numpy(), ref["qA"])
+    assert np.array_equal(A.unpack_codes(qW, N, K, A.OPERAND_WEIGHT).cpu().numpy(), ref["qW"])
+    assert np.array_equal(A.scales_to_natural(sA, M, G).cpu().numpy().view(np.uint16), ref["sA"].view(np.uint16))
+    assert np.array_equal(A.scales_to_natural(sW, N, G).cpu().numpy().view(np.uint16), ref["sW"].view(np.uint16))
+    Y = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=torch.float32 if out_f32 else torch.float16, opts=o)
+    # a second and third call on one (self-cleaning) workspace must give the same answer
+    ws = A.make_workspace(M, N, K, g, opts=o)
+    Y2 = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=Y.dtype, workspace=ws, opts=o)
+    Y3 = A.w4a4_gemm(qA, sA, qW, sW, M, N, K, g, out_dtype=Y.dtype, workspace=ws, opts=o)
+    if sums == "all":
+        P = A.debug_group_sums(qA, qW, M, N, K, g, opts=o).cpu().numpy()
+        assert np.array_equal(P, O.group_sums(ref["qA"], ref["qW"], g))
+    elif sums is not None:
+        m0, m1, n0, n1 = sums
+        P = A.debug_group_sums(qA, qW, M, N, K, g, m0=m0, m1=m1, n0=n0, n1=n1, opts=o).cpu().numpy()
+        assert np.array_equal(P, O.group_sums(ref["qA"][m0:m1], ref["qW"][n0:n1], g))
+    torch.cuda.synchronize()
     for y in (Y, Y2, Y3):
         check_output(y.cpu().numpy(), ref["Y64"], ref["T"], G, not out_f32)
     if ws is not None:
         assert int(ws.count_nonzero()) == 0      # workspace left zero-filled
     return ref
+
+
+PAIR, DECODE = 1, 0   # apex4_debug_opts.kernel
 
 
 def test_gemm_config0(A):
@@ -148,12 +152,18 @@ def test_gemm_config0(A):
 
 
 @pytest.mark.parametrize("g", [32, 64, 128, 256, 512])
-@pytest.mark.parametrize("dispatch", [(16, 0, -1), (16, 1, -1), (16, 1, 3), (32, 0, -1), (32, 1, 5),
-                                      (64, 1, -1), (128, 0, 1), (128, 1, 7), (256, 0, -1), (256, 1, 3)])
-def test_gemm_config0_all_dispatches(A, g, dispatch):
-    """Same problem through every token-tile width, whole-tile and stream-K work distribution and
-    several grid sizes (dispatch = (tile width, stream-K, CTAs))."""
-    run_gemm_case(A, 16, 256, 512, g, seed=0, fixed=True, dispatch=dispatch)
+@pytest.mark.parametrize("opts", [dict(kernel=PAIR), dict(kernel=PAIR, split=1, grid=3), dict(kernel=PAIR, split=1, grid=1),
+                                  dict(kernel=PAIR, pair_tokens=128, split=1, grid=2), dict(kernel=PAIR, pair_tokens=192),
+                                  dict(kernel=DECODE), dict(kernel=DECODE, grid=3, decode_batch=2)])
+def test_gemm_config0_all_dispatches(A, g, opts):
+    """Same problem through both kernels, every token-tile width of the pair kernel, whole-tile and
+    stream-K work distribution and several grid sizes."""
+    if opts["kernel"] == DECODE and g == 256:
+        with pytest.raises(A.Apex4Error) as e:      # the decode kernel does not cover 128 < g < K (K = 512 here)
+            run_gemm_case(A, 16, 256, 512, g, seed=0, fixed=True, opts=opts)
+        assert e.value.status == A.ERR_INVALID_ARG
+        return
+    run_gemm_case(A, 16, 256, 512, g, seed=0, fixed=True, opts=opts)
 
 
 @pytest.mark.parametrize("M,N,K,g", [(1, 256, 512, 128), (4, 264, 1024, 128), (17, 136, 384, 32),
@@ -164,55 +174,66 @@ def test_gemm_ragged_and_multi_tile(A, M, N, K, g):
 
 
 @pytest.mark.parametrize("M,N,K", [(1, 8, 128), (16, 136, 1024), (17, 1000, 512), (32, 8192, 256),
-                                   (33, 264, 2048), (48, 520, 1024), (64, 456, 1536), (5, 64, 28672)])
-@pytest.mark.parametrize("grid", [-1, 1, 3])
+                                   (20, 264, 2048), (31, 520, 1024), (5, 64, 28672)])
+@pytest.mark.parametrize("grid", [0, 1, 3])
 def test_gemm_decode_kernels(A, M, N, K, grid):
-    """The decode-regime kernels (g = 128: bulk-copy staged for one or two m16 token tiles -- the automatic
-    choice for M <= 32 --, register-ring for three or four, reachable through the test hook) on ragged N,
-    row ranges that straddle 128-row tiles, K from one k-block to the longest supported row, and several
-    grid sizes (rows per CTA / batches per CTA)."""
-    # automatic dispatch: the decode kernel up to M = 32, CTA pairs on 64-token tiles above
-    assert A.debug_get_dispatch(M, N, K, 128)[0] == (0 if M <= 32 else 256)
-    run_gemm_case(A, M, N, K, 128, seed=300 + M, dispatch=(0, -1, grid))
+    """The decode-regime kernel at g = 128 (one or two m16 token tiles) on ragged N, row ranges that
+    straddle 128-row tiles, K from one k-block to the longest supported row, and several grid sizes
+    (rows per CTA / batches per CTA)."""
+    assert A.debug_get_dispatch(M, N, K, 128)[0] == DECODE      # the automatic choice for M <= 32
+    run_gemm_case(A, M, N, K, 128, seed=300 + M, opts=dict(kernel=DECODE, grid=grid))
+
+
+def test_dispatch_above_decode_range(A):
+    """32 < M: CTA pairs (64-token tiles up to M = 64); asking for the decode kernel there is an error."""
+    assert A.debug_get_dispatch(33, 264, 2048, 128)[:2] == (PAIR, 64)
+    assert A.debug_get_dispatch(64, 8192, 8192, 128)[:2] == (PAIR, 64)
+    with pytest.raises(A.Apex4Error):
+        A.debug_get_dispatch(33, 264, 2048, 128, opts=A.debug_opts(kernel=DECODE))
+    run_gemm_case(A, 33, 264, 2048, 128, seed=333)
+    run_gemm_case(A, 64, 456, 1536, 128, seed=364)
 
 
 @pytest.mark.parametrize("M,N,K", [(1, 8, 256), (16, 136, 1024), (17, 1000, 512), (32, 8192, 256),
                                    (20, 264, 2048), (5, 64, 28672)])
-@pytest.mark.parametrize("grid", [-1, 1, 3])
+@pytest.mark.parametrize("grid", [0, 1, 3])
 def test_gemm_decode_per_channel(A, M, N, K, grid):
     """Per-channel decode (M <= 32, g = K): the decode kernel keeps INT32 partial sums through the k loop
     and the cross-warp reduction, so the group sum is exact and rounded once (R12)."""
-    assert A.debug_get_dispatch(M, N, K, K)[0] == 0
-    run_gemm_case(A, M, N, K, K, seed=700 + M, dispatch=(0, -1, grid))
-    run_gemm_case(A, M, N, K, K, seed=700 + M, dispatch=(0, -1, grid), out_f32=True, sums=None)
+    assert A.debug_get_dispatch(M, N, K, K)[0] == DECODE
+    run_gemm_case(A, M, N, K, K, seed=700 + M, opts=dict(kernel=DECODE, grid=grid))
+    run_gemm_case(A, M, N, K, K, seed=700 + M, opts=dict(kernel=DECODE, grid=grid), out_f32=True, sums=None)
 
 
 @pytest.mark.parametrize("M,N,K,g", [(1, 8, 256, 32), (16, 136, 1024, 32), (17, 1000, 512, 64), (32, 8192, 256, 32),
                                      (20, 264, 2048, 64), (9, 4096, 11008, 32), (5, 64, 28672, 64)])
-@pytest.mark.parametrize("grid", [-1, 3])
+@pytest.mark.parametrize("grid", [0, 3])
 def test_gemm_decode_fine_groups(A, M, N, K, g, grid):
     """Decode at g = 32 / 64 (M <= 32): every MMA (pair of MMAs) of the decode kernel covers exactly one
     group and is scaled on its own; group sums bit-exact, outputs inside the tolerance, FP16 and FP32."""
-    assert A.debug_get_dispatch(M, N, K, g)[0] == 0
-    run_gemm_case(A, M, N, K, g, seed=800 + M, dispatch=(0, -1, grid))
-    run_gemm_case(A, M, N, K, g, seed=800 + M, dispatch=(0, -1, grid), out_f32=True, sums=None)
+    assert A.debug_get_dispatch(M, N, K, g)[0] == DECODE
+    run_gemm_case(A, M, N, K, g, seed=800 + M, opts=dict(kernel=DECODE, grid=grid))
+    run_gemm_case(A, M, N, K, g, seed=800 + M, opts=dict(kernel=DECODE, grid=grid), out_f32=True, sums=None)
 
 
 @pytest.mark.parametrize("M,N,K,g", [(40, 264, 512, 128), (64, 520, 1024, 32), (100, 520, 1024, 128),
                                      (130, 304, 1024, 512), (300, 520, 1024, 1024), (200, 264, 2048, 64)])
-@pytest.mark.parametrize("dispatch", [(256 + 64, 0, -1), (256 + 128, 0, -1), (256 + 192, 0, -1),
-                                      (256 + 64, 1, 3), (256 + 128, 1, 5)])
-def test_gemm_pair_tile_widths(A, M, N, K, g, dispatch):
-    """The CTA-pair kernel at its three token-tile widths (64 / 128 / 192; the hook value is 256 + width),
-    whole tiles and stream-K, FP16 and FP32 output, on ragged shapes."""
-    run_gemm_case(A, M, N, K, g, seed=500 + M, dispatch=dispatch)
-    run_gemm_case(A, M, N, K, g, seed=500 + M, dispatch=dispatch, out_f32=True, sums=None)
+@pytest.mark.parametrize("opts", [dict(kernel=PAIR, pair_tokens=64, split=0), dict(kernel=PAIR, pair_tokens=128, split=0),
+                                  dict(kernel=PAIR, pair_tokens=192, split=0),
+                                  dict(kernel=PAIR, pair_tokens=64, split=1, grid=3),
+                                  dict(kernel=PAIR, pair_tokens=128, split=1, grid=5),
+                                  dict(kernel=PAIR, pair_tokens=192, split=1, grid=2)])
+def test_gemm_pair_tile_widths(A, M, N, K, g, opts):
+    """The CTA-pair kernel at its three token-tile widths (64 / 128 / 192), whole tiles and stream-K,
+    FP16 and FP32 output, on ragged shapes."""
+    run_gemm_case(A, M, N, K, g, seed=500 + M, opts=opts)
+    run_gemm_case(A, M, N, K, g, seed=500 + M, opts=opts, out_f32=True, sums=None)
 
 
 def test_gemm_decode_f32_and_large_group_routing(A):
-    run_gemm_case(A, 16, 256, 1024, 128, seed=7, out_f32=True, dispatch=(0, -1, -1))
+    run_gemm_case(A, 16, 256, 1024, 128, seed=7, out_f32=True, opts=dict(kernel=DECODE))
     # groups larger than a k-block keep one rounding per group: the pair kernel handles them
-    assert A.debug_get_dispatch(16, 256, 1024, 256)[0] == 256
+    assert A.debug_get_dispatch(16, 256, 1024, 256)[:2] == (PAIR, 64)
     run_gemm_case(A, 16, 256, 1024, 256, seed=8)
 
 
@@ -322,11 +343,9 @@ def test_error_codes_on_device(A):
     assert e.value.status == A.ERR_UNSUPPORTED_SHAPE
     q, s, _ = A.quantize_act(x, 128)
     with pytest.raises(A.Apex4Error) as e:     # stream-K dispatch without a workspace
-        A.lib().apex4_debug_set_dispatch(16, 1, 2)
-        try:
-            st = A.lib().apex4_w4a4_gemm(q.data_ptr(), s.data_ptr(), q.data_ptr(), s.data_ptr(), x.data_ptr(),
-                                         0, 16, 128, 512, 128, 0, 0, None, 0, None)
-            A._check(st, "gemm")
-        finally:
-            A.debug_set_dispatch(-1, -1, -1)
+        import ctypes
+        o = A.debug_opts(kernel=PAIR, split=1, grid=2)
+        st = A.lib().apex4_w4a4_gemm_ex(q.data_ptr(), s.data_ptr(), q.data_ptr(), s.data_ptr(), x.data_ptr(),
+                                        0, 16, 512, 512, 128, 0, 0, None, 0, None, ctypes.byref(o))
+        A._check(st, "gemm")
     assert e.value.status == A.ERR_WORKSPACE
