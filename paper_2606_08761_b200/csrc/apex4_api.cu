@@ -64,7 +64,6 @@ int resolve_g(int K, int group_size, int gran, int layer) {
 
 struct Dispatch {
   int kernel;  // 0 = decode (weight-stream) kernel, 1 = CTA-pair tcgen05 kernel
-  int bias;    // pair kernel: magic-biased accumulators (g <= 128)
   int split;   // pair kernel: stream-K work distribution (needs the workspace)
   int grid;    // CTAs (decode) or CTA pairs (pair kernel)
   int upt, kbu, tiles_m, tiles_n;
@@ -110,14 +109,12 @@ bool choose_dispatch(int M, int N, int K, int g, const apex4_debug_opts& o, Disp
   const int KB = K / kBlockK;
   d.kbu = g > kBlockK ? g / kBlockK : 1;   // indivisible k unit: a whole group, at least a k-block
   d.upt = KB / d.kbu;
-  d.bias = g <= kBlockK;
   const bool dec_ok = decode_supported(M, K, g);
   if (o.kernel == 0 && !dec_ok) return false;
   if (o.kernel > 1 || o.kernel < -1) return false;
   d.kernel = o.kernel >= 0 ? o.kernel : (dec_ok ? 0 : 1);
   if (d.kernel == 0) {
     // a CTA owns a contiguous range of 8-row row blocks and all of K; no workspace
-    d.bias = 0;
     d.mt = (M + 15) / 16;
     d.tiles_m = 1;
     d.tiles_n = (N + 7) / 8;
@@ -154,7 +151,7 @@ size_t counters_bytes(const Dispatch& d) {
 }
 
 cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
-  const cudaError_t e = d.kernel == 1 ? launch_gemm_pair(p, d.bias, dump, d.grid, st) : launch_gemv(p, d.mt, dump, d.grid, st);
+  const cudaError_t e = d.kernel == 1 ? launch_gemm_pair(p, dump, d.grid, st) : launch_gemv(p, d.mt, dump, d.grid, st);
   if (e != cudaSuccess && getenv("APEX4_VERBOSE"))
     fprintf(stderr, "apex4: GEMM launch (kernel %d, grid %d) failed: %s\n", d.kernel, d.grid, cudaGetErrorString(e));
   return e;

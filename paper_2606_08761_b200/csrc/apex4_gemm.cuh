@@ -36,7 +36,7 @@ constexpr int kPairTokens = 192;   // tokens per CTA-pair tile (the widest; 128 
 // Tensor-bound regime (apex4_gemm_pair.cu): CTA pairs (cluster of 2, cta_group::2), work tile = 256
 // weight rows x p.pair_nt tokens; tiles_m / tiles_n / counters are in units of pair tiles (counters: two per
 // tile, one per CTA of the pair).  npairs <= gemm_max_pairs().
-cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st);
+cudaError_t launch_gemm_pair(const GemmParams& p, bool dump, int npairs, cudaStream_t st);
 int gemm_max_pairs();
 
 // Decode regime (apex4_gemv.cu): M <= 32 at g = 32 / 64 / 128 or per-channel, no workspace.  tiles_n = 8-row

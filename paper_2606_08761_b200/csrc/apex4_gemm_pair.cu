@@ -1,750 +1,25 @@
-// apex4_gemm_pair.cu -- a2..a7 of the hot path (every shape but decode M <= 32 at g = 128): the W4A4
-// group-dequant GEMM of Eq. 8 on a CTA PAIR (cluster of 2, tcgen05 cta_group::2).
-//
-// A pair owns a 256 (weight rows n) x NT (tokens m) output tile; NT = 192 below, 128 / 64 are the same
-// kernel instantiated for small M (Tile<NT>).  CTA r of the pair holds weight
-// rows 128 r .. 128 r + 127 of the tile on its 128 TMEM lanes and supplies 96 of the 192 token rows
-// of every MMA from its own shared memory, so per SM and k-block (K = 128) only 8 KB of packed
-// weights and 6 KB of packed activations are fetched, widened and read by the tensor core
-// (shared-memory read bandwidth is the scarce resource, profiles/r1_ubench_b200.md).
-//
-// Why 192 tokens: (1) TMEM holds two full 192-column accumulator buffers plus four 32-column
-// weight-operand stages (2 x 192 + 4 x 32 = 512), so the MMA of group g+1 runs while the epilogue
-// drains group g; (2) an epilogue thread keeps 96 FP32 running sums, which leaves registers for a
-// true software prefetch of the next TMEM chunk (with 128 sums ptxas serialised load and arithmetic).
-//
-// Roles (W = 1 or 2 widener warpgroups, template parameter, see Warps<> below; the launch register
-// count x threads is the pool that setmaxnreg redistributes: control 32, wideners 40, epilogue 184-200):
-//   warps 0..4W-1  wideners : k-blocks dealt alternately between the warpgroups.  INT4 -> INT8 (x16).
-//                          Thread r widens weight row r in registers and stores it to TMEM; 96 token
-//                          rows are widened smem -> smem into the 128B-swizzled UMMA layout.  One elected
-//                          arrive per warp on the LEADER's operand barrier.  FP16 -> FP32 scale prep.
-//   next 8 warps   epilogue : warpgroup h owns tokens 96 h .. 96 h + 95.  tcgen05.ld.32x32b.x16: a thread
-//                          holds one weight row (its TMEM lane) x 16 consecutive tokens per chunk; this
-//                          shape sustains ~1.4 x the TMEM read rate of 16x256b (profiles/r1_ubench_b200.md);
-//                          chunk c+1 is in flight while chunk c is in the FMA pipe.  Two FFMA2 per element
-//                          pair: fma(f, sW/256, -49152 sW) = P sW rounded once (magic-biased accumulators),
-//                          then fma with the two token scales into the FP32 sums.
-//   then           producer : 1-D bulk async copies (UBLKCP) of this CTA's packed INT4 rows + FP16 scales
-//   then           MMA      : leader CTA only; tcgen05.mma cta_group::2 kind::i8, M = 256, N = 192, K = 32,
-//                          A (weights) from TMEM, B (tokens) from shared memory; tcgen05.commit
-//                          multicast to both CTAs.  Producer and MMA loops run warp-uniform with one
-//                          elected lane issuing (operands in uniform registers, no divisions).
-#include <type_traits>
-
-#include "apex4_gemm.cuh"
-#include "apex4_layout.cuh"
-#include "apex4_ptx.cuh"
+// apex4_gemm_pair.cu -- host side of the CTA-pair kernel (apex4_gemm_pair.cuh): picks the granularity MODE
+// instantiation and answers how many CTA pairs can be resident.
+#include "apex4_gemm_pair.cuh"
 
 namespace apex4 {
 
-namespace pair {
-
-constexpr uint32_t kMagicBits = 0x4B400000u;   // float 12582912 = 1.5 * 2^23
-constexpr int kEpiWGs = 2;          // epilogue warpgroups (each owns kNT / kEpiWGs token columns)
-constexpr int kEpiWarps = 4 * kEpiWGs;
-constexpr int kAccBufs = 2;
-constexpr int kOpStages = 4;        // widened operand stages (TMEM A + smem B)
-constexpr int kPkStages = 6;        // packed (bulk copy) stages
-constexpr int kScfSlots = 8;
-constexpr int kTmemA0 = 384;        // first TMEM column of the A-operand stages
-constexpr int kPkWBytes = kBlobBytes;             // 128 weight rows of a k-block
-constexpr int kPkSWBytes = 4 * 256;               // up to 4 groups per k-block, 128 FP16 each
-constexpr int kPkSABytes = 2 * 4 * 256;           // the (up to) two 128-token blobs the tile touches
-constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs;
-static_assert((kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
-static_assert((kOpStages & (kOpStages - 1)) == 0, "stage index wraps with a mask");
-
-// Everything that depends on the token width NT of the pair tile (MMA N = accumulator buffer width):
-// 192 in the tensor-bound regime, 128 / 64 where M would leave most of a 192-token tile empty.
-template <int NT>
-struct Tile {
-  static constexpr int kNT = NT;
-  static constexpr int kHalf = NT / 2;                  // token rows per CTA (its half of the B operand)
-  static constexpr int kEpiCols = NT / kEpiWGs;         // accumulator columns per epilogue warpgroup
-  static constexpr int kChunks = kEpiCols / 16;         // 16-column TMEM chunks per epilogue thread
-  static constexpr int kTokIters = kHalf / 32;          // 16-byte token pieces per widener thread
-  static constexpr int kPkABytes = kHalf * kRowBytes;   // packed token rows of a k-block
-  static constexpr int kPkStageBytes = kPkWBytes + kPkABytes + kPkSWBytes + kPkSABytes;
-  static constexpr int kI8StageBytes = kHalf * kBlockK; // widened tokens: [kHalf rows][128 B]
-  static constexpr int kScfSlotBytes = kTileRows * 8 + NT * 4 + 256;   // {a,b} per row, sA per column (padded)
-  static constexpr int kStoreBytes = kEpiCols * 64;     // per epilogue warp: [kEpiCols m][32 n] FP16 output staging
-  static constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
-                                    kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + kEpiWarps * kStoreBytes;
-  static_assert(NT % 64 == 0 && NT <= kPairTokens, "token width");
-  static_assert(kAccBufs * NT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
-  static_assert(kI8StageBytes % 1024 == 0 && kPkStageBytes % 16 == 0, "alignment");
-  static_assert(kSmemBytes <= 232448, "shared memory");
-  static_assert(NT % (16 * kEpiWGs) == 0, "epilogue warpgroups own whole 16-column chunks");
-};
-
-// Warp layout for WWG widener warpgroups.  With one, the wideners of a CTA run one k-block at a time:
-// fewer warps polling barriers and competing for issue slots, which is what the epilogue-heavy fine
-// granularities want (g <= 128: 903 vs 949 us at 8192^3); with two, k-blocks are dealt alternately and
-// the bulk copy -> widen -> MMA chain is shorter, which is what counts once the epilogue is rare
-// (per-channel, M = 4096, N = K = 8192: 252 vs 294 us).  The register pool is threads x launch
-// registers (<= 64 K), redistributed by setmaxnreg: control 32, wideners 40, the rest to the epilogue.
-template <int WWG>
-struct Warps {
-  static constexpr int kWidenWGs = WWG;                     // k-blocks dealt alternately
-  static constexpr int kEpiWarp0 = 4 * WWG;                 // first epilogue warp
-  static constexpr int kCtlWarp0 = kEpiWarp0 + kEpiWarps;   // producer warp; the MMA warp follows
-  static constexpr int kThreads = 32 * (kCtlWarp0 + 4);     // warps are allocated in fours: two control warps idle
-  static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8 > 120 ? 120 : (65536 / kThreads) / 8 * 8;
-  static constexpr int kRegsCtl = 32, kRegsWiden = 40;
-  static constexpr int kRegsEpi = ((kThreads * kLaunchRegs - 128 * kRegsCtl - 128 * WWG * kRegsWiden) / (128 * kEpiWGs)) / 8 * 8;
-  static_assert((WWG & (WWG - 1)) == 0, "k-blocks are dealt with a mask");
-  static_assert(128 * kRegsCtl + 128 * WWG * kRegsWiden + 128 * kEpiWGs * kRegsEpi <= kThreads * kLaunchRegs, "registers");
-  static_assert(kRegsEpi <= 232 && kThreads <= 1024, "register / thread limits");
-};
-// widener warpgroups for a resolved group size
-inline int widen_wgs(int g) {
-#ifdef APEX4_PAIR_FORCE_WWG   // tuning builds only
-  return APEX4_PAIR_FORCE_WWG;
-#else
-  return g <= kBlockK ? 1 : 2;
-#endif
-}
-
-struct Work {
-  int nt, mt;      // pair tile: 256 weight rows x NT tokens
-  int kb0, kb1;
-  int partial, units;
-};
-struct WorkIter {
-  long long u, u1;
-  int i;
-};
-__device__ __forceinline__ void work_begin(const GemmParams& p, WorkIter& it, int cp, int npairs) {
-  it.i = 0;
-  const long long total = static_cast<long long>(p.tiles_m) * p.tiles_n * p.upt;
-  it.u = total * cp / npairs;
-  it.u1 = total * (cp + 1) / npairs;
-}
-// Tiles are numbered token-tile fastest: pairs that run together share weight tiles in L2.
-__device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Work& w, int cp, int npairs) {
-#ifdef APEX4_PAIR_EMPTY   // tuning builds only: launch + set-up + teardown cost
-  return false;
-#endif
-  int tile;
-  if (p.split == 0) {
-    tile = cp + it.i * npairs;
-    if (tile >= p.tiles_m * p.tiles_n) return false;
-    ++it.i;
-    w.kb0 = 0; w.kb1 = p.K / kBlockK; w.partial = 0; w.units = p.upt;
-  } else {
-    if (it.u >= it.u1) return false;
-    tile = static_cast<int>(it.u / p.upt);
-    const int off = static_cast<int>(it.u - static_cast<long long>(tile) * p.upt);
-    const long long left = it.u1 - it.u;
-    const int n = static_cast<int>(left < p.upt - off ? left : p.upt - off);
-    w.kb0 = off * p.kbu; w.kb1 = (off + n) * p.kbu; w.partial = (n != p.upt); w.units = n;
-    it.u += n;
-  }
-  w.mt = tile % p.tiles_m;
-  w.nt = tile / p.tiles_m;
-  return true;
-}
-
-}  // namespace pair
-
-using namespace pair;
-
-template <bool BIAS, bool DUMP, int WWG, int NT>
-__global__ void __cluster_dims__(2, 1, 1) __maxnreg__(Warps<WWG>::kLaunchRegs)
-    w4a4_gemm_pair_kernel(const GemmParams p) {
-  using L = Warps<WWG>;
-  using T = Tile<NT>;
-  constexpr int kNT = T::kNT, kHalf = T::kHalf, kEpiCols = T::kEpiCols, kChunks = T::kChunks;
-  constexpr int kPkABytes = T::kPkABytes, kPkStageBytes = T::kPkStageBytes, kI8StageBytes = T::kI8StageBytes;
-  constexpr int kScfSlotBytes = T::kScfSlotBytes, kStoreBytes = T::kStoreBytes, kTokIters = T::kTokIters;
-  constexpr int kWidenWGs = L::kWidenWGs, kEpiWarp0 = L::kEpiWarp0, kCtlWarp0 = L::kCtlWarp0;
-  constexpr int kRegsCtl = L::kRegsCtl, kRegsWiden = L::kRegsWiden, kRegsEpi = L::kRegsEpi;
-  extern __shared__ uint8_t smem_raw[];
-  // opaque: otherwise ptxas re-derives the base (S2R SR_CgaCtaId + 4 integer ops) in front of every
-  // barrier wait and shared-memory access instead of keeping it in a register
-  uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  asm volatile("" : "+r"(smem_base));
-  uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-
-  constexpr uint32_t offI8 = 0;
-  constexpr uint32_t offPk = offI8 + kOpStages * kI8StageBytes;
-  constexpr uint32_t offScf = offPk + kPkStages * kPkStageBytes;
-  constexpr uint32_t offBar = offScf + kScfSlots * kScfSlotBytes;
-  constexpr uint32_t offTmemPtr = offBar + kNumBars * 8;
-  constexpr uint32_t offMagic = offTmemPtr + 64;       // 8 words of the magic bias (see epilogue)
-  constexpr uint32_t offStore = (offMagic + 64 + 15) / 16 * 16;   // 8 x kStoreBytes output staging
-  auto bar = [&](int i) { return smem_base + offBar + 8u * i; };
-  constexpr int bPkFull = 0, bPkEmpty = bPkFull + kPkStages, bOpFull = bPkEmpty + kPkStages,
-                bOpEmpty = bOpFull + kOpStages, bScfFull = bOpEmpty + kOpStages,
-                bScfEmpty = bScfFull + kScfSlots, bAccFull = bScfEmpty + kScfSlots,
-                bAccEmpty = bAccFull + kAccBufs;
-
-  // warp index through a shuffle from lane 0: tells the compiler it is warp-uniform, so addresses derived
-  // from it (TMEM lane quarter, barrier and stage addresses) live in uniform registers (no R2UR per use)
-  const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
-  int lane = threadIdx.x & 31;
-  asm volatile("" : "+r"(lane));                // no S2R SR_TID.X inside the loops
-  const uint32_t rank = cluster_ctarank();      // 0 = leader
-  const int cp = blockIdx.x >> 1;               // pair index
-  const int npairs = gridDim.x >> 1;
-  const int g = p.g;
-  const int gpk = g < kBlockK ? kBlockK / g : 1;        // groups per k-block (1, 2, 4)
-  const int kbpg = g > kBlockK ? g / kBlockK : 1;       // k-blocks per group
-  // Scale-slot hand-shake.  At g = 128 (one group per k-block) it is implied by the operand / accumulator
-  // barriers and skipped -- every mbarrier wait costs ~250 clk even when the phase is already complete:
-  //  * full:  the wideners write slot k before they publish operand stage k, the MMA of group k is
-  //           issued after that, so "accumulator k full" implies "scales k written";
-  //  * empty: the widener of k-block k has waited for operand stage k % 4 = MMA k-4 done, which was
-  //           issued after all epilogue warps released accumulator k-6, i.e. had finished group k-8,
-  //           the previous user of slot k % 8.
-  const bool scf_sync = g != kBlockK;
-
-  if (threadIdx.x == 0) {
-    for (int i = 0; i < kPkStages; ++i) { mbar_init(bar(bPkFull + i), 1); mbar_init(bar(bPkEmpty + i), 128); }
-    // operand stage full: one elected arrive per widener warp of BOTH CTAs, on the leader's barrier
-    for (int i = 0; i < kOpStages; ++i) { mbar_init(bar(bOpFull + i), 8); mbar_init(bar(bOpEmpty + i), 1); }
-    for (int i = 0; i < kScfSlots; ++i) { mbar_init(bar(bScfFull + i), 128); mbar_init(bar(bScfEmpty + i), kEpiWarps); }
-    // accumulator buffer empty: one elected arrive per epilogue warp of BOTH CTAs, on the leader's barrier
-    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 2 * kEpiWarps); }
-    fence_mbar_init();
-  }
-  if (threadIdx.x < 8) reinterpret_cast<volatile uint32_t*>(smem_gen + offMagic)[threadIdx.x] = kMagicBits;
-  if (warp == kCtlWarp0 + 1) tmem_alloc_pair<512>(smem_base + offTmemPtr);
-  tc_fence_before();
-  __syncthreads();
-  cluster_sync_all();       // barriers of both CTAs initialised before any remote arrive / multicast
-  tc_fence_after();
-  const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + offTmemPtr);
-  if (tmem_base != 0) __trap();   // the whole TMEM (512 columns) is ours: lane 0, column 0
-
-  WorkIter wit;
-  Work w;
-  work_begin(p, wit, cp, npairs);
-  auto stamp = [&](int ev, uint32_t k) {   // debug timeline: compiled in with -DAPEX4_TIMELINE only
-#ifdef APEX4_TIMELINE
-    if (p.tl != nullptr && blockIdx.x == 0 && k < 64) p.tl[ev * 64 + k] = clock64();
-#endif
-  };
-
-  // =========================================================================== control warps
-  if (warp >= kCtlWarp0) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsCtl));
-    // ------------------------------------------------------------------------- producer
-    // The whole warp runs the loop on warp-uniform values, one elected lane issues the copies;
-    // source pointers advance by a blob per k-block (no division, no 64-bit multiplies).
-    if (warp == kCtlWarp0) {
-      const bool el = elect_one();
-      const int n_blobs = round_up(p.N, kTileRows) / kTileRows;
-      const int m_blobs = round_up(p.M, kTileRows) / kTileRows;
-      const uint32_t sc_bytes = gpk * 256;
-      const size_t row_pitch = static_cast<size_t>(p.K / kBlockK) * kBlobBytes;   // bytes per blob row
-      const size_t srow_pitch = static_cast<size_t>(p.G) * kTileRows;               // FP16 scales per blob row
-      uint32_t kbc = 0, s = 0, pkpar = 0;
-      while (work_next(p, wit, w, cp, npairs)) {
-        const int wblob = 2 * w.nt + static_cast<int>(rank);
-        const bool has_w = wblob < n_blobs;
-        // this CTA's 96 token rows: up to two pieces of consecutive blobs
-        const int t0 = w.mt * kNT + static_cast<int>(rank) * kHalf;
-        const int ab0 = t0 >> 7, ar0 = t0 & 127;
-        const int n1 = ab0 < m_blobs ? min(kHalf, kTileRows - ar0) : 0;
-        const int n2 = (ab0 + 1 < m_blobs) ? kHalf - min(kHalf, kTileRows - ar0) : 0;
-        // token scales: the two blobs the 192-token tile touches
-        const int sb0 = (w.mt * kNT) >> 7;
-        const int s_blobs = min((((w.mt * kNT) & 127) + kNT > kTileRows) ? 2 : 1, m_blobs - sb0);
-        const int gfirst0 = g < kBlockK ? w.kb0 * gpk : w.kb0 / kbpg;
-        const uint8_t* wsrc = p.qW + wblob * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes;
-        const uint8_t* asrc = p.qA + ab0 * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes + ar0 * kRowBytes;
-        const __half* swsrc = p.sW + wblob * srow_pitch + static_cast<size_t>(gfirst0) * kTileRows;
-        const __half* sasrc = p.sA + sb0 * srow_pitch + static_cast<size_t>(gfirst0) * kTileRows;
-        const uint32_t bytes_data = (has_w ? kBlobBytes : 0) + (n1 + n2) * kRowBytes;
-        const uint32_t bytes_scales = sc_bytes * ((has_w ? 1 : 0) + s_blobs);
-        int kig = 0;
-        for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-          mbar_wait(bar(bPkEmpty + s), ((pkpar >> s) & 1) ^ 1);
-          pkpar ^= 1u << s;
-          const uint32_t st = smem_base + offPk + s * kPkStageBytes;
-          const uint32_t full = bar(bPkFull + s);
-          const bool has_scales = !DUMP && kig == 0;   // the dump of the integer sums takes no scales (null pointers)
-          if (el) {
-            stamp(0, kbc);
-            mbar_arrive_expect_tx(full, bytes_data + (has_scales ? bytes_scales : 0));
-            if (has_w) bulk_g2s(st, wsrc, kBlobBytes, full);
-            if (n1 > 0) bulk_g2s(st + kPkWBytes, asrc, n1 * kRowBytes, full);
-            if (n2 > 0)   // rows 0.. of the next blob
-              bulk_g2s(st + kPkWBytes + n1 * kRowBytes, asrc + row_pitch - ar0 * kRowBytes, n2 * kRowBytes, full);
-            if (has_scales) {
-              if (has_w) bulk_g2s(st + kPkWBytes + kPkABytes, swsrc, sc_bytes, full);
-              if (s_blobs > 0) bulk_g2s(st + kPkWBytes + kPkABytes + kPkSWBytes, sasrc, sc_bytes, full);
-              if (s_blobs > 1)
-                bulk_g2s(st + kPkWBytes + kPkABytes + kPkSWBytes + sc_bytes, sasrc + srow_pitch, sc_bytes, full);
-            }
-          }
-          wsrc += kBlobBytes;
-          asrc += kBlobBytes;
-          if (has_scales) { swsrc += sc_bytes / 2; sasrc += sc_bytes / 2; }
-          kig = (kig == kbpg - 1) ? 0 : kig + 1;
-          s = (s == kPkStages - 1) ? 0 : s + 1;
-        }
-      }
-    }
-    // ------------------------------------------------------------------------- debug observer
-#ifdef APEX4_TIMELINE
-    else if (warp == kCtlWarp0 + 2 && p.tl != nullptr && blockIdx.x == 0) {
-      uint32_t kbc = 0, s = 0, par = 0;
-      while (work_next(p, wit, w, cp, npairs)) {
-        for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-          if (kbc < 64) { mbar_wait(bar(bPkFull + s), (par >> s) & 1); if (lane == 0) stamp(14, kbc); }
-          par ^= 1u << s;
-          s = (s == kPkStages - 1) ? 0 : s + 1;
-        }
-      }
-    }
-#endif
-    // ------------------------------------------------------------------------- MMA issuer (leader)
-    // Whole warp, warp-uniform values, one elected lane issues.  No division, no 64-bit descriptor
-    // arithmetic, stage / buffer parities kept as bit masks: the first version of this loop took
-    // ~2000 clk per k-block and was the bottleneck of the kernel (round 1).
-    else if (warp == kCtlWarp0 + 1 && rank == 0) {
-      const bool el = elect_one();
-      const uint32_t desc_lo0 = (((smem_base + offI8) & 0x3FFFFu) >> 4) | (1u << 16);
-      uint32_t kbc = 0, t = 0, oppar = 0, accpar = 0, buf0 = 0;
-      while (work_next(p, wit, w, cp, npairs)) {
-        int kig = 0;                                     // k-block inside the group
-        for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-          mbar_wait(bar(bOpFull + t), (oppar >> t) & 1);
-          oppar ^= 1u << t;
-          tc_fence_after();
-          if (el) stamp(4, kbc);
-          const bool first = kig == 0;
-          const bool last = kig == kbpg - 1;
-          const uint32_t a_tm = kTmemA0 + 32 * t;        // the 512-column allocation starts at column 0
-          const uint32_t blo = desc_lo0 + t * (kI8StageBytes >> 4);
-          auto issue = [&](auto gpk_c) {
-            constexpr int GPK = decltype(gpk_c)::value;
-            constexpr int KS = 4 / GPK;
-#pragma unroll
-            for (int sub = 0; sub < GPK; ++sub) {
-              const uint32_t buf = (buf0 + sub) & 1;     // one accumulator buffer per group
-              if (first) {
-                mbar_wait(bar(bAccEmpty + buf), (accpar >> buf) & 1);
-                accpar ^= 1u << buf;
-                tc_fence_after();
-              }
-#pragma unroll
-              for (int ks = 0; ks < KS; ++ks) {
-                const int kq = sub * KS + ks;            // K=32 slice of the k-block
-                if (el) {
-                  if (BIAS || ks != 0) mma_i8_ts_pair_lohi<true, kNT>(buf * kNT, a_tm + 8 * kq, blo + 2 * kq, 1u);
-                  else mma_i8_ts_pair_lohi<false, kNT>(buf * kNT, a_tm + 8 * kq, blo + 2 * kq, first ? 0u : 1u);
-                }
-              }
-              if (last && el) tc_commit_pair(bar(bAccFull + buf), 3);
-            }
-          };
-          if (gpk == 1) issue(std::integral_constant<int, 1>{});
-          else if (gpk == 2) issue(std::integral_constant<int, 2>{});
-          else issue(std::integral_constant<int, 4>{});
-          if (el) tc_commit_pair(bar(bOpEmpty + t), 3);
-          if (el) stamp(5, kbc);
-          t = (t + 1) & (kOpStages - 1);
-          if (last) { buf0 = (buf0 + gpk) & 1; kig = 0; } else { ++kig; }
-        }
-      }
-    }
-  }
-  // =========================================================================== wideners
-  // Two warpgroups, k-blocks dealt alternately: one warp per SM sub-partition running a k-block's
-  // LDS -> LOP -> STS/STTM -> fence chain is latency-bound; two in flight overlap each other's drains.
-  else if (warp < kEpiWarp0) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsWiden));
-    const int wwg = warp >> 2;                          // widener warpgroup
-    const int r = threadIdx.x & 127;                    // weight row of this CTA's blob = TMEM lane
-    const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
-    const uint32_t wsw = (r >> 1) & 3;                  // chunk-slot swizzle of the packed row (PW4)
-    const uint32_t flip = ((lane >> 2) & 1) * 16;       // order of the two 16-byte stores: spreads them over the banks
-    constexpr uint32_t kMask = 0xF0F0F0F0u;
-    uint32_t kbc = 0, gc = 0, s = 0, t = 0, pkpar = 0, oppar = 0;
-    while (work_next(p, wit, w, cp, npairs)) {
-      const int sa_off = (w.mt * kNT) & 127;            // tile token 0 inside its first scale blob
-      int kig = 0;
-      for (int kb = w.kb0; kb < w.kb1; ++kb, ++kbc) {
-        const bool starts_group = kig == 0;
-        kig = (kig == kbpg - 1) ? 0 : kig + 1;
-        const uint32_t s_cur = s, t_cur = t;
-        s = (s == kPkStages - 1) ? 0 : s + 1;
-        t = (t + 1) & (kOpStages - 1);
-        const uint32_t pk_ph = (pkpar >> s_cur) & 1, op_ph = (oppar >> t_cur) & 1;
-        pkpar ^= 1u << s_cur;
-        oppar ^= 1u << t_cur;
-        if (static_cast<int>(kbc & (kWidenWGs - 1)) != wwg) {   // the other warpgroup's k-block
-          if (starts_group) gc += gpk;
-          continue;
-        }
-        mbar_wait(bar(bPkFull + s_cur), pk_ph);
-        if (r == 0) stamp(1, kbc);
-        const uint32_t pk_addr = smem_base + offPk + s_cur * kPkStageBytes;
-        uint32_t wv[8];
-        lds128(pk_addr + r * kRowBytes + ((0 ^ wsw) << 4), wv[0], wv[1], wv[2], wv[3]);
-        lds128(pk_addr + r * kRowBytes + ((1 ^ wsw) << 4), wv[4], wv[5], wv[6], wv[7]);
-        mbar_wait(bar(bOpEmpty + t_cur), op_ph ^ 1);
-        tc_fence_after();
-        if (r == 0) stamp(2, kbc);
-        // ---- weights: packed row r (64 bytes) -> 32 INT8 words -> TMEM columns of stage t
-#pragma unroll
-        for (int hh = 0; hh < 2; ++hh) {
-          uint32_t o[16];
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              o[8 * j + i] = rotl4(wv[4 * j + i]) & kMask;
-              o[8 * j + 4 + i] = wv[4 * j + i] & kMask;
-            }
-          }
-          if (hh == 0) {
-            lds128(pk_addr + r * kRowBytes + ((2 ^ wsw) << 4), wv[0], wv[1], wv[2], wv[3]);
-            lds128(pk_addr + r * kRowBytes + ((3 ^ wsw) << 4), wv[4], wv[5], wv[6], wv[7]);
-          }
-          tmem_st_32x16(tmem_base + lane_addr + kTmemA0 + 32 * t_cur + 16 * hh, o);
-        }
-        if (r == 0) stamp(9, kbc);
-        // ---- tokens: 96 rows x 4 packed chunks; byte offset o -> INT8 offsets 2o (lo), 2o+16 (hi)
-        {
-          uint32_t av[4 * kTokIters];
-#pragma unroll
-          for (int x = 0; x < kTokIters; ++x)
-            lds128(pk_addr + kPkWBytes + (r + 128 * x) * 16, av[4 * x], av[4 * x + 1], av[4 * x + 2], av[4 * x + 3]);
-          const uint32_t dst0 = smem_base + offI8 + t_cur * kI8StageBytes;
-#pragma unroll
-          for (int x = 0; x < kTokIters; ++x) {
-            const uint32_t dst = dst0 + (r + 128 * x) * 32;
-            const uint32_t l0 = rotl4(av[4 * x]) & kMask, h0 = av[4 * x] & kMask;
-            const uint32_t l1 = rotl4(av[4 * x + 1]) & kMask, h1 = av[4 * x + 1] & kMask;
-            const uint32_t l2 = rotl4(av[4 * x + 2]) & kMask, h2 = av[4 * x + 2] & kMask;
-            const uint32_t l3 = rotl4(av[4 * x + 3]) & kMask, h3 = av[4 * x + 3] & kMask;
-            if (flip) {
-              sts128(dst + 16, h0, h1, h2, h3);
-              sts128(dst, l0, l1, l2, l3);
-            } else {
-              sts128(dst, l0, l1, l2, l3);
-              sts128(dst + 16, h0, h1, h2, h3);
-            }
-          }
-        }
-        // ---- scales of the groups that start in this k-block: FP16 -> FP32, BEFORE the stage is published:
-        // at g = 128 the epilogue takes "accumulator full" as "scales written" (see scf_sync)
-        if (starts_group) {
-          const uint8_t* pk = smem_gen + offPk + s_cur * kPkStageBytes;
-          const __half* sWh = reinterpret_cast<const __half*>(pk + kPkWBytes + kPkABytes);
-          const __half* sAh = sWh + kPkSWBytes / 2;     // [blob 0/1][sub][128]
-          for (int sub = 0; sub < gpk; ++sub, ++gc) {
-            const int q = gc % kScfSlots;
-            if (scf_sync) mbar_wait(bar(bScfEmpty + q), ((gc / kScfSlots) & 1) ^ 1);
-            float* dstf = reinterpret_cast<float*>(smem_gen + offScf + q * kScfSlotBytes);
-            const float sw = __half2float(sWh[sub * kTileRows + r]);
-            // a = sW / 256 (the operands are 16 q each); b = -12582912 * a removes the magic bias
-            reinterpret_cast<float2*>(dstf)[r] = make_float2(sw * 0.00390625f, sw * -49152.0f);
-            // token scales, in tile order (an epilogue thread reads the 16 of a chunk as four 16-byte vectors)
-#pragma unroll
-            for (int x = 0; x < 2; ++x) {
-              const int col = r + 128 * x;                       // token of the tile
-              if (col < kNT) {
-                const int mm = sa_off + col;                     // row in the tile's two scale blobs
-                dstf[2 * kTileRows + col] = __half2float(sAh[((mm >> 7) * gpk + sub) * kTileRows + (mm & 127)]);
-              }
-            }
-            if (scf_sync) mbar_arrive(bar(bScfFull + q));
-          }
-        }
-        // ---- publish stage t: one elected arrive per warp on the leader's barrier
-        if (r == 0) stamp(10, kbc);
-        fence_proxy_async_smem();
-        if (r == 0) stamp(11, kbc);
-        tmem_st_wait();
-        if (r == 0) stamp(12, kbc);
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(bar(bOpFull + t_cur), 0);
-        if (r == 0) stamp(3, kbc);
-        mbar_arrive(bar(bPkEmpty + s_cur));
-        if (r == 0) stamp(13, kbc);
-      }
-    }
-  }
-  // =========================================================================== epilogue
-  else {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsEpi));
-    const int h = (warp - kEpiWarp0) >> 2;              // warpgroup = slice of kEpiCols token columns
-    const int lq = warp & 3;                            // TMEM lane quarter this warp may access
-    const int epi_tid = threadIdx.x - 32 * kEpiWarp0;
-    const uint32_t lane_addr = static_cast<uint32_t>(lq * 32) << 16;
-    const int row0 = lq * 32 + lane;                    // weight row of the CTA's blob = TMEM lane
-    // per-thread address parts of the group loop, made opaque so that ptxas keeps them in registers
-    // instead of re-deriving them from %tid in every group (11 S2R + ~40 integer ops per group)
-    const uint32_t tm_rd = lane_addr + h * kEpiCols;                                   // + buf * kNT
-    uint32_t ab_off = offScf + row0 * 8;                                      // {a, b} of row row0
-    uint32_t sa_off = offScf + kTileRows * 8 + (h * kEpiCols) * 4;            // token scales (+ 64 c)
-    asm volatile("" : "+r"(ab_off), "+r"(sa_off));   // tm_rd stays warp-uniform (uniform registers)
-    // the magic bias in 8 registers, read through a volatile load so that ptxas keeps them resident
-    // instead of re-materialising 16 constants per tcgen05.st (IMAD.MOV on the FMA pipe)
-    uint32_t mg[8];
-    {
-      const uint32_t ma = smem_base + offMagic;
-      asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(mg[0]), "=r"(mg[1]), "=r"(mg[2]), "=r"(mg[3]) : "r"(ma));
-      asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(mg[4]), "=r"(mg[5]), "=r"(mg[6]), "=r"(mg[7]) : "r"(ma + 16));
-    }
-    // completion #0 of the accEmpty barriers: both buffers start out holding the magic bias
-#pragma unroll
-    for (int b = 0; b < kAccBufs; ++b) {
-      if (BIAS) {
-#pragma unroll
-        for (int c = 0; c < kEpiCols; c += 8) tmem_st_32x8(tmem_base + lane_addr + b * kNT + h * kEpiCols + c, mg);
-        tmem_st_wait();
-      }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + b), 0);
-    }
-
-    uint32_t gc = 0, item = 0;
-    while (work_next(p, wit, w, cp, npairs)) {
-      if (epi_tid == 0) stamp(15, item * 4);
-      const int nkb = w.kb1 - w.kb0;
-      const int ngroups = g < kBlockK ? nkb * gpk : nkb / kbpg;
-      uint64_t acc[8 * kChunks];                        // FP32 pairs: tokens 2 x, 2 x + 1 of the slice
-#pragma unroll
-      for (int i = 0; i < 8 * kChunks; ++i) acc[i] = 0ull;
-      const int n_glob0 = (2 * w.nt + static_cast<int>(rank)) * kTileRows + row0;
-      const int m_glob0 = w.mt * kNT + h * kEpiCols;        // + 16 c + j
-
-      for (int gi = 0; gi < ngroups; ++gi, ++gc) {
-        const int slot = gc % kScfSlots;
-        const uint32_t buf = gc & 1;
-        if (scf_sync) mbar_wait(bar(bScfFull + slot), (gc / kScfSlots) & 1);
-        mbar_wait(bar(bAccFull + buf), (gc >> 1) & 1);
-        const uint32_t scf = smem_base + slot * kScfSlotBytes;
-        {
-          // ---- this thread = weight row row0 (TMEM lane), 16 consecutive tokens per chunk
-          float af, bf;
-          unpack_f2(lds64(scf + ab_off), af, bf);
-          const uint64_t a2 = pack_f2(af, af), b2 = pack_f2(bf, bf);
-          const uint32_t sAf = scf + sa_off;   // + 64 c
-          tc_fence_after();
-          if (epi_tid == 0) stamp(6, gc);
-          const uint32_t tb = tm_rd + buf * kNT;
-          uint32_t v[2][16];
-          uint64_t sq[8];                                  // token scales of the chunk, as pairs
-          tmem_ld_32x16(tb, v[0]);
-#pragma unroll
-          for (int c = 0; c < kChunks; ++c) {
-            uint32_t* vc = v[c & 1];
-            // the scales of chunk c (those of chunk c - 1 have been consumed): in flight during the wait
-            lds_2x64(sAf + 64 * c, sq[0], sq[1]);
-            lds_2x64(sAf + 64 * c + 16, sq[2], sq[3]);
-            lds_2x64(sAf + 64 * c + 32, sq[4], sq[5]);
-            lds_2x64(sAf + 64 * c + 48, sq[6], sq[7]);
-            tmem_ld_wait16(vc);
-            if (c < kChunks - 1) tmem_ld_32x16(tb + 16 * (c + 1), v[(c + 1) & 1]);
-            if constexpr (BIAS) {
-              tmem_st_32x8(tb + 16 * c, mg);
-              tmem_st_32x8(tb + 16 * c + 8, mg);
-            }
-            if (c == kChunks - 1) {                        // buffer fully read (and re-armed): hand it back
-              if constexpr (BIAS) tmem_st_wait();
-              tc_fence_before();
-              __syncwarp();
-              if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + buf), 0);
-            }
-            if constexpr (DUMP) {
-              const int gamma = (g < kBlockK ? w.kb0 * gpk : w.kb0 / kbpg) + gi;
-#pragma unroll
-              for (int j = 0; j < 16; ++j) {
-                const int m = m_glob0 + 16 * c + j;
-                const int n = n_glob0;
-                if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1) {
-                  const uint32_t x = vc[j];
-                  const int32_t raw = static_cast<int32_t>(BIAS ? x - kMagicBits : x);
-                  p.P_out[(static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gamma] = raw >> 8;
-                }
-              }
-            }
-#pragma unroll
-            for (int jj = 0; jj < 8; ++jj) {
-              uint64_t t0;
-              if constexpr (BIAS) {
-                t0 = fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2);
-              } else {
-                t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[2 * jj])), __int2float_rn(static_cast<int>(vc[2 * jj + 1]))), a2);
-              }
-              acc[c * 8 + jj] = fma2(t0, sq[jj], acc[c * 8 + jj]);   // tokens 16 c + 2 jj, + 1
-            }
-          }
-        }
-        if (scf_sync) {
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar(bScfEmpty + slot));
-        }
-        if (epi_tid == 0) stamp(7, gc);
-      }
-
-      // ---- a7 (cast + store) or a6 (cross-pair reduce through the FP32 workspace)
-      if (epi_tid == 0) stamp(15, item * 4 + 1);
-      if (p.Y != nullptr) {
-        auto store_tile = [&]() {
-          if (!p.out_f32) {
-            // FP16 output: the warp's 32 (n) x 96 (m) sub-tile goes through a private 6 KB shared-memory
-            // tile [m][32 n] (16-byte part p of row m stored at p ^ ((m >> 1) & 3)), then out as 16-byte
-            // row pieces: 12 STG.128 per thread instead of 96 STG.U16 with 64-bit address arithmetic
-            // (the store phase was 10-12 % of the config-1 GEMM time)
-            const uint32_t stg = smem_base + offStore + (warp - kEpiWarp0) * kStoreBytes;
-#pragma unroll
-            for (int x = 0; x < 8 * kChunks; ++x) {       // tokens m = 2 x, 2 x + 1 of the warpgroup's slice, n = lane
-              float f0, f1;
-              unpack_f2(acc[x], f0, f1);
-              const uint32_t a0 = stg + (2 * x) * 64 + (((lane >> 3) ^ (x & 3)) << 4) + 2 * (lane & 7);
-              asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0), "h"(__half_as_ushort(__float2half_rn(f0))) : "memory");
-              asm volatile("st.shared.b16 [%0], %1;" ::"r"(a0 + 64), "h"(__half_as_ushort(__float2half_rn(f1))) : "memory");
-            }
-            __syncwarp();
-            const int n = (2 * w.nt + static_cast<int>(rank)) * kTileRows + lq * 32 + (lane & 3) * 8;
-            __half* ybase = static_cast<__half*>(p.Y) + n;
-#pragma unroll
-            for (int ps = 0; ps < kEpiCols / 8; ++ps) {
-              const int row = ps * 8 + (lane >> 2);
-              uint32_t x0, x1, x2, x3;
-              lds128(stg + row * 64 + (((lane & 3) ^ ((row >> 1) & 3)) << 4), x0, x1, x2, x3);
-              const int m = w.mt * kNT + h * kEpiCols + row;
-              if (m < p.M && n < p.N)
-                *reinterpret_cast<uint4*>(ybase + static_cast<size_t>(m) * p.N) = make_uint4(x0, x1, x2, x3);
-            }
-            __syncwarp();
-            return;
-          }
-          float* y = static_cast<float*>(p.Y);      // FP32 output: lanes = consecutive n, coalesced rows
-          if (n_glob0 < p.N) {
-#pragma unroll
-            for (int x = 0; x < 8 * kChunks; ++x) {
-              float f0, f1;
-              unpack_f2(acc[x], f0, f1);
-              const int m = m_glob0 + 2 * x;
-              if (m < p.M) y[static_cast<size_t>(m) * p.N + n_glob0] = f0;
-              if (m + 1 < p.M) y[static_cast<size_t>(m + 1) * p.N + n_glob0] = f1;
-            }
-          }
-        };
-        if (!w.partial) {
-          store_tile();
-        } else {
-          // a6: FP32 partial sums meet in the workspace ("inter-SM global reduction").  The
-          // workspace holds every CTA tile in FRAGMENT order -- [tile][CTA][j = 0..23][thread][4 floats] --
-          // so a partial tile is 24 fully coalesced red.global.add.v4.f32 per thread (not 96 scalar
-          // atomics), and the CTA that completes the tile reads it back with the same thread mapping,
-          // leaves it zero-filled, casts and stores.
-          float* wst = p.ws + static_cast<size_t>((w.nt * p.tiles_m + w.mt) * 2 + static_cast<int>(rank)) * (kTileRows * kNT) +
-                       epi_tid * 4;
-#pragma unroll
-          for (int j = 0; j < 4 * kChunks; ++j) {
-            float f0, f1, f2, f3;
-            unpack_f2(acc[2 * j], f0, f1);
-            unpack_f2(acc[2 * j + 1], f2, f3);
-            asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(wst + j * (128 * kEpiWarps)), "f"(f0),
-                         "f"(f1), "f"(f2), "f"(f3)
-                         : "memory");
-          }
-          __threadfence();
-          if (epi_tid == 0) stamp(15, item * 4 + 2);
-          int* flag = reinterpret_cast<int*>(smem_gen + offTmemPtr + 8);
-          asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
-          if (epi_tid == 0) {
-            const int tile = (w.nt * p.tiles_m + w.mt) * 2 + static_cast<int>(rank);
-            const int prev = atomicAdd(p.counters + tile, w.units);
-            const int done = (prev + w.units == p.upt);
-            *flag = done;
-            if (done) p.counters[tile] = 0;
-          }
-          asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
-          const int done = *flag;
-          asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");   // flag may be rewritten by the next item
-          if (done) {
-            __threadfence();
-#pragma unroll
-            for (int j = 0; j < 4 * kChunks; ++j) {       // all loads first, then the zero stores
-              const float4 x = __ldcg(reinterpret_cast<const float4*>(wst + j * (128 * kEpiWarps)));
-              acc[2 * j] = pack_f2(x.x, x.y);
-              acc[2 * j + 1] = pack_f2(x.z, x.w);
-            }
-#pragma unroll
-            for (int j = 0; j < 4 * kChunks; ++j) __stcg(reinterpret_cast<float4*>(wst + j * (128 * kEpiWarps)), make_float4(0.f, 0.f, 0.f, 0.f));
-            store_tile();
-          }
-        }
-      }
-      if (epi_tid == 0) stamp(15, item * 4 + 3);
-      ++item;
-    }
-    tc_fence_before();
-  }
-
-  // ---- teardown: nobody leaves while the peer may still signal this CTA's barriers or read its
-  // shared memory / TMEM through the pair MMA
-  cluster_sync_all();
-  if (warp == kCtlWarp0 + 1) {
-    tc_fence_after();
-    tmem_dealloc_pair<512>(tmem_base);
+cudaError_t launch_gemm_pair(const GemmParams& p, bool dump, int npairs, cudaStream_t st) {
+  switch (gran_mode(p.g)) {
+    case 0: return launch_pair_mode<0>(p, dump, npairs, st);
+    case 1: return launch_pair_mode<1>(p, dump, npairs, st);
+    case 2: return launch_pair_mode<2>(p, dump, npairs, st);
+    default: return launch_pair_mode<3>(p, dump, npairs, st);
   }
 }
 
-// ------------------------------------------------------------------------------------ launcher
-template <bool BIAS, bool DUMP, int WWG, int NT>
-static cudaError_t launch_pair_one(const GemmParams& p, int npairs, cudaStream_t st) {
-  auto kern = w4a4_gemm_pair_kernel<BIAS, DUMP, WWG, NT>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<NT>::kSmemBytes);
-  if (e != cudaSuccess) return e;
-  kern<<<2 * npairs, Warps<WWG>::kThreads, Tile<NT>::kSmemBytes, st>>>(p);
-  return cudaGetLastError();
-}
-template <int WWG, int NT>
-static cudaError_t launch_pair_w(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
-  if (bias) return dump ? launch_pair_one<true, true, WWG, NT>(p, npairs, st) : launch_pair_one<true, false, WWG, NT>(p, npairs, st);
-  return dump ? launch_pair_one<false, true, WWG, NT>(p, npairs, st) : launch_pair_one<false, false, WWG, NT>(p, npairs, st);
-}
-template <int NT>
-static cudaError_t launch_pair_nt(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
-  return widen_wgs(p.g) == 1 ? launch_pair_w<1, NT>(p, bias, dump, npairs, st) : launch_pair_w<2, NT>(p, bias, dump, npairs, st);
-}
-
-cudaError_t launch_gemm_pair(const GemmParams& p, bool bias, bool dump, int npairs, cudaStream_t st) {
-  switch (p.pair_nt) {
-    case 64: return launch_pair_nt<64>(p, bias, dump, npairs, st);
-    case 128: return launch_pair_nt<128>(p, bias, dump, npairs, st);
-    case kPairTokens: return launch_pair_nt<kPairTokens>(p, bias, dump, npairs, st);
-    default: return cudaErrorInvalidValue;
-  }
-}
+// declared here, defined in apex4_gemm_pair_m3.cu (it needs a kernel symbol for the occupancy query)
+int gemm_max_pairs_query();
 
 // CTA pairs that can be resident at once (one per TPC); queried once
 int gemm_max_pairs() {
   static int pairs = 0;
-  if (pairs == 0) {
-    auto kern = w4a4_gemm_pair_kernel<true, false, 2, kPairTokens>;   // one CTA per SM whatever the layout
-    int n = 0;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(2 * 74);
-    cfg.blockDim = dim3(Warps<2>::kThreads);
-    cfg.dynamicSmemBytes = Tile<kPairTokens>::kSmemBytes;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<kPairTokens>::kSmemBytes) != cudaSuccess ||
-        cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) {
-      cudaGetLastError();
-      n = 74;   // B200: 148 SMs, one CTA pair per TPC
-    }
-    pairs = n;
-  }
+  if (pairs == 0) pairs = gemm_max_pairs_query();
   return pairs;
 }
 

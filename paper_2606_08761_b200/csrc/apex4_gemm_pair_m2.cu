@@ -1,0 +1,7 @@
+// apex4_gemm_pair_m2.cu -- the CTA-pair kernel of apex4_gemm_pair.cuh instantiated for granularity MODE 2
+// (g = 32); one translation unit per mode so that they compile in parallel.
+#include "apex4_gemm_pair.cuh"
+
+namespace apex4 {
+APEX4_PAIR_INSTANTIATE(2)
+}  // namespace apex4
