@@ -292,3 +292,96 @@ def test_policy_table():
         assert O.resolve_group_size(K, layer, O.POLICY_BASELINE_MIX) == 128
     for layer in (O.LAYER_Q, O.LAYER_K, O.LAYER_O, O.LAYER_GATE, O.LAYER_UP, O.LAYER_GATE_UP, O.LAYER_QKV):
         assert O.resolve_group_size(K, layer, O.POLICY_PAPER_MIX) == K
+
+
+# ----------------------------------------------------------------- T, the tolerance, the FP32-ordered sum
+def test_pin_T_and_output_tolerance():
+    """T (second return of dequant_gemm) and output_tolerance set the bar of every GPU output check, so they
+    are pinned to numbers typed from the hand derivation in tests/golden/p1_worked_example.txt:
+    g = 4: terms 1.0*0.125*69 = 8.625 and 0.28564453125*0.25*(-24) = -1.7138671875
+           T = 8.625 + 1.7138671875 = 10.3388671875
+           tol (FP32 out) = 1e-3 * 6.9111328125 + (2+2) * 2^-23 * 10.3388671875
+                          = 0.0069111328125 + 4.76837158203125e-07 * 10.3388671875 = 0.00691606276855...
+           FP16 out adds one subnormal ulp 2^-24 = 5.9604644775390625e-08."""
+    fx = read_kv_fixture("p1_worked_example.txt")
+    A = f16(fx["A"])[None, :]
+    W = f16(fx["W"])[None, :]
+    qA, sA = O.quantize(A, 4)
+    qW, sW = O.quantize(W, 4)
+    Y64, T = O.dequant_gemm(qA, sA, qW, sW, 4)
+    assert T.shape == (1, 1) and T[0, 0] == 10.3388671875
+    tol32 = O.output_tolerance(Y64, T, 2, False)[0, 0]
+    tol16 = O.output_tolerance(Y64, T, 2, True)[0, 0]
+    assert abs(tol32 - 0.006916062768548727) < 1e-17
+    assert abs(tol16 - (0.006916062768548727 + 5.9604644775390625e-08)) < 1e-17
+    # a x1000 (or /1000) mistake in either term would move the bound by far more than this
+    assert 0.0069 < tol32 < 0.00693 and tol16 > tol32
+    # per-channel (g = 8): one term, T = |Y| = 8.5, tol = 8.5e-3 + 3 * 2^-23 * 8.5
+    qA8, sA8 = O.quantize(A, 8)
+    qW8, sW8 = O.quantize(W, 8)
+    Y8, T8 = O.dequant_gemm(qA8, sA8, qW8, sW8, 8)
+    assert T8[0, 0] == 8.5
+    assert abs(O.output_tolerance(Y8, T8, 1, False)[0, 0] - (0.0085 + 3 * 8.5 / 8388608.0)) < 1e-17
+    # P3: every term is positive, so T == Y64 exactly, for every g
+    X1 = np.ones((2, 512), dtype=np.float16)
+    for g in (32, 128, 512):
+        r = O.w4a4_linear(X1, X1, g)
+        assert np.array_equal(r["T"], r["Y64"])
+    # cancellation: equal and opposite groups give Y = 0 but T = 2 |term| (the bound must not vanish)
+    Xc = np.ones((1, 64), dtype=np.float16)
+    Wc = np.ones((1, 64), dtype=np.float16)
+    Wc[0, 32:] = -1
+    rc = O.w4a4_linear(Xc, Wc, 32)
+    term = 49 * 32 * (585.0 / 4096.0) ** 2
+    assert rc["Y64"][0, 0] == 0.0 and rc["T"][0, 0] == 2 * term
+    assert O.output_tolerance(rc["Y64"], rc["T"], 2, False)[0, 0] == 4 * 2.0 ** -23 * 2 * term
+
+
+def _rn_f32(x):
+    """Round an exact rational to binary32 (ties to even) with integer arithmetic only."""
+    from fractions import Fraction
+    x = Fraction(x)
+    if x == 0:
+        return Fraction(0)
+    s = -1 if x < 0 else 1
+    x = abs(x)
+    e = 0
+    while x >= 2 ** 24:
+        x /= 2
+        e += 1
+    while x < 2 ** 23:
+        x *= 2
+        e -= 1
+    n, rem = divmod(x.numerator, x.denominator)
+    twice = 2 * rem
+    if twice > x.denominator or (twice == x.denominator and n % 2 == 1):
+        n += 1
+    return s * Fraction(n) * Fraction(2) ** e
+
+
+def test_pin_f32_ordered_sum():
+    """dequant_gemm_f32_order against (i) the hand example, where every step is exact in binary32:
+    fma(69, 0.125, 0) = 8.625, fma(-24, 0.0714111328125, 8.625) = 6.9111328125; (ii) an exact-rational
+    restatement of acc = rn32(P * (sA * sW) + acc) on a small random problem."""
+    from fractions import Fraction
+    fx = read_kv_fixture("p1_worked_example.txt")
+    A = f16(fx["A"])[None, :]
+    W = f16(fx["W"])[None, :]
+    qA, sA = O.quantize(A, 4)
+    qW, sW = O.quantize(W, 4)
+    Y32 = O.dequant_gemm_f32_order(qA, sA, qW, sW, 4)
+    assert Y32.dtype == np.float32 and float(Y32[0, 0]) == 6.9111328125
+    rng = np.random.default_rng(12)
+    X = (rng.standard_normal((3, 256)) * 3).astype(np.float16)
+    Wm = (rng.standard_normal((4, 256)) * 0.02).astype(np.float16)
+    g = 32
+    r = O.w4a4_linear(X, Wm, g)
+    Y32 = O.dequant_gemm_f32_order(r["qA"], r["sA"], r["qW"], r["sW"], g)
+    for m in range(3):
+        for n in range(4):
+            acc = Fraction(0)
+            for gam in range(256 // g):
+                P = sum(int(a) * int(b) for a, b in zip(r["qA"][m, gam * g:(gam + 1) * g], r["qW"][n, gam * g:(gam + 1) * g]))
+                s = Fraction(float(r["sA"][m, gam])) * Fraction(float(r["sW"][n, gam]))     # 22 bits: exact in binary32
+                acc = _rn_f32(P * s + acc)
+            assert Fraction(float(Y32[m, n])) == acc, (m, n)
