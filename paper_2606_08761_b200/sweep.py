@@ -50,7 +50,9 @@ def gemm_bytes(M, N, K, g):
     return N * K / 2 + 2 * N * G + M * K / 2 + 2 * M * G + 2 * M * N
 
 
-def time_shape(M, N, K, g, dev, cublas=True):
+def time_shape(M, N, K, g, dev, cublas=True, with_quant=False):
+    """with_quant: also time quantize_act + GEMM captured together (what a W4A4 linear costs next to an FP16
+    GEMM, which needs no online quantizer) -> "us_with_quant"."""
     per_set = N * K / 2 + M * K / 2
     nsets = int(max(1, min(8, 2 * L2_BYTES // per_set + 1)))
     sets = []
@@ -72,6 +74,17 @@ def time_shape(M, N, K, g, dev, cublas=True):
            "tops": round(2.0 * M * N * K / us * 1e-6, 1),
            "gbs": round(gemm_bytes(M, N, K, g) / us * 1e-3, 1),
            "kernel": ("gemv", "pair")[apex4.debug_get_dispatch(M, N, K, g)[0]]}
+    if with_quant:
+        nx = int(max(2, min(8, 2 * L2_BYTES // (2 * M * K) + 1)))
+        xs = [torch.randn(M, K, device=dev, dtype=torch.float16) for _ in range(nx)]
+        qa0, sa0 = sets[0][0], sets[0][1]
+
+        def run_q(i):
+            apex4.quantize_act(xs[i % nx], g, q=qa0, s=sa0)
+            apex4.w4a4_gemm(qa0, sa0, sets[i % nsets][2], sets[i % nsets][3], M, N, K, g, out=Y, workspace=ws)
+
+        out["us_with_quant"] = round(_graph_time_us(run_q, max(nx, nsets)), 2)
+        del xs
     del sets
     if cublas:
         nb = int(max(1, min(4, 2 * L2_BYTES // (2 * N * K) + 1)))
@@ -80,7 +93,9 @@ def time_shape(M, N, K, g, dev, cublas=True):
         c = torch.empty((M, N), device=dev, dtype=torch.float16)
         cu = _graph_time_us(lambda i: torch.matmul(a, bs[i].t(), out=c), nb)
         out["cublas_fp16_us"] = round(cu, 2)
-        out["speedup_vs_cublas_fp16"] = round(cu / us, 2)
+        out["speedup_vs_cublas_fp16"] = round(cu / us, 2)                      # GEMM alone
+        if with_quant:
+            out["speedup_vs_cublas_fp16_with_quant"] = round(cu / out["us_with_quant"], 2)
         del bs
     torch.cuda.empty_cache()
     return out
