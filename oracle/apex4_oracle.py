@@ -20,8 +20,11 @@ Parity pins (tests/test_oracle_pins.py): hand-worked K=8 example
 (tests/golden/p1_worked_example.txt), scale bit patterns, all-ones closed form,
 scaled identity, FP64 dequantise-then-matmul identity, invariants, exhaustive
 exact-integer restatement of the rounding decision over all FP16 inputs,
-integer-matmul special case.  Every function below has at least one such pin;
-nothing here is "parity unpinned".
+integer-matmul special case; T / output_tolerance / dequant_gemm_f32_order on the
+hand example and an exact-rational restatement; rmsnorm / silu_mul on hand values,
+invariants, an exact-rational (integer sqrt) restatement and a 50-digit decimal
+evaluation of every finite FP16 gate.  Every function below has at least one
+such pin; nothing here is "parity unpinned".
 
 Natural layouts used here (the C-ABI's device layouts differ; the binding
 converts):  X[R,K] float16, codes q[R,K] int8 in [-8,7], scales S[R,G] float16
@@ -190,6 +193,50 @@ def w4a4_linear(X, W, g: int):
     qW, sW = quantize(W, g)
     Y64, T = dequant_gemm(qA, sA, qW, sW, g)
     return dict(qA=qA, sA=sA, qW=qW, sW=sW, Y64=Y64, T=T, Y16=to_f16(Y64))
+
+
+# --------------------------------------------------------------------------
+# F1/F2  producers of the quantizer's input ("quantized online", PAPER.md:150, 256 -- the paper
+#        does not say what feeds the quantizer; in a Llama / Qwen block it is RMSNorm (QKV, gate/up inputs)
+#        and SiLU(gate) * up (down_proj input).  Neither is in the paper's equations: the readings below are
+#        DESIGN.md R17 / R18.  The fused CUDA calls apex4_rmsnorm_quantize / apex4_silu_mul_quantize must
+#        produce exactly quantize(rmsnorm(...), g) / quantize(silu_mul(...), g).)
+# --------------------------------------------------------------------------
+def rmsnorm(X: np.ndarray, gamma: np.ndarray, eps: float) -> np.ndarray:
+    """R17.  y[m,k] = fp16_rn( (x[m,k] * inv[m]) * gamma[k] ), evaluated in IEEE binary32:
+        ss[m]  = sum_k x[m,k]^2                 exact (every square of an FP16 value is exact in binary32 and
+                                                 the sum of K <= 32768 of them is exact in binary64, in any order)
+        ms[m]  = float32( ss[m] / K )           one rounding
+        inv[m] = 1.0f / sqrtf( ms[m] + eps )    IEEE add, sqrt, divide (each correctly rounded)
+        y      = fp16_rn( fmul(fmul(x, inv), gamma) )
+    X[M,K] float16, gamma[K] float16, eps a binary32 value.  Returns float16 [M,K]."""
+    X = np.asarray(X)
+    gamma = np.asarray(gamma)
+    assert X.dtype == np.float16 and gamma.dtype == np.float16 and X.ndim == 2 and gamma.shape == (X.shape[1],)
+    K = X.shape[1]
+    assert K <= 32768
+    x64 = X.astype(np.float64)
+    ss = np.sum(x64 * x64, axis=1)                                   # exact
+    ms = (ss / np.float64(K)).astype(np.float32)
+    inv = np.float32(1.0) / np.sqrt(ms + np.float32(eps), dtype=np.float32)
+    y32 = (X.astype(np.float32) * inv[:, None]) * gamma.astype(np.float32)[None, :]
+    assert y32.dtype == np.float32
+    with np.errstate(over="ignore"):
+        return y32.astype(np.float16)
+
+
+def silu_mul(gate: np.ndarray, up: np.ndarray) -> np.ndarray:
+    """R18.  y = fp16_rn( silu(gate) * up ), silu(g) = g / (1 + exp(-g)): the real-valued product rounded ONCE to
+    FP16 (evaluated in binary64, whose 2^-52 error can move an FP16 rounding only within 2^-40 of a tie).
+    gate, up float16 of equal shape.  Returns float16."""
+    gate = np.asarray(gate)
+    up = np.asarray(up)
+    assert gate.dtype == np.float16 and up.dtype == np.float16 and gate.shape == up.shape
+    g = gate.astype(np.float64)
+    with np.errstate(over="ignore"):
+        s = g / (1.0 + np.exp(-g))                                   # exp(-g) = inf for g < -709 never happens: |g| <= 65504 -> s = -0.0
+        s = np.where(np.isfinite(s), s, 0.0)
+        return (s * up.astype(np.float64)).astype(np.float16)
 
 
 # --------------------------------------------------------------------------

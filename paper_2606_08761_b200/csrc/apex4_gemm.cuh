@@ -31,6 +31,23 @@ struct GemmParams {
   long long* tl;       // -DAPEX4_TIMELINE builds only: clock64 stamps of CTA 0, [event][64]; else unused
 };
 
+// Launch with programmatic stream serialization (PDL): the kernel may start while its predecessor on the
+// stream drains; it calls griddep_wait() (apex4_ptx.cuh) before it touches anything the predecessor wrote.
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 constexpr int kPairTokens = 192;   // tokens per CTA-pair tile (the widest; 128 / 64 where M is small)
 
 // Tensor-bound regime (apex4_gemm_pair.cu): CTA pairs (cluster of 2, cta_group::2), work tile = 256

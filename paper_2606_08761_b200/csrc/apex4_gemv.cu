@@ -158,7 +158,23 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     tx = (n1 + n2) * kRowBytes + Cfg::kABytes + ((CH || DUMP) ? 0 : GS * (n1 + n2) * 2 + Cfg::kSABytes);
   };
   if (rb0 < rb1 && nkw > 0) batch_setup();
-  auto issue_next = [&]() {                             // copies of one stage
+  // The activation side of a stage (packed token rows + token scales): what the PREVIOUS kernel on the stream
+  // (the online quantizer) writes.  The weight side is constant, so the first stages' weight copies are issued
+  // before griddep_wait() and stream in while the predecessor drains (programmatic dependent launch).
+  auto issue_tokens = [&](uint32_t st, uint32_t full, const uint8_t* aq_, const __half* sq_) {
+    if (el) {
+      bulk_g2s(st + Cfg::kWBytes, aq_, Cfg::kABytes, full);
+      if constexpr (!CH && !DUMP) {
+#pragma unroll
+        for (int gs = 0; gs < GS; ++gs)
+          bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes + gs * (MT * 32), sq_ + gs * kTileRows, MT * 32, full);
+      }
+    }
+  };
+  const uint8_t* aq_pre[kStages] = {};
+  const __half* sq_pre[kStages] = {};
+  int n_pre = 0;
+  auto issue_next = [&](bool tokens_now) {              // copies of one stage
     if (ib0 >= rb1 || nkw == 0) return;
     const uint32_t st = my_stage0 + islot * Cfg::kStageBytes;
     const uint32_t full = my_bar0 + 8 * islot;
@@ -166,16 +182,21 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       mbar_arrive_expect_tx(full, tx);
       bulk_g2s(st, w1, n1b, full);
       if (n2b > 0) bulk_g2s(st + n1b, w2, n2b, full);
-      bulk_g2s(st + Cfg::kWBytes, aq, Cfg::kABytes, full);
       if constexpr (!CH && !DUMP) {
 #pragma unroll
         for (int gs = 0; gs < GS; ++gs) {               // 2 bytes per row and group
           const uint32_t dsw = st + Cfg::kWBytes + Cfg::kABytes + gs * (RBB * 16);
           bulk_g2s(dsw, s1 + gs * kTileRows, n1b >> 5, full);
           if (n2b > 0) bulk_g2s(dsw + (n1b >> 5), s2 + gs * kTileRows, n2b >> 5, full);
-          bulk_g2s(st + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes + gs * (MT * 32), sq + gs * kTileRows, MT * 32, full);
         }
       }
+    }
+    if (tokens_now) {
+      issue_tokens(st, full, aq, sq);
+    } else {                                            // prologue: after griddep_wait()
+      aq_pre[n_pre] = aq;
+      sq_pre[n_pre] = sq;
+      ++n_pre;
     }
     w1 += kBlobBytes; w2 += kBlobBytes; aq += kBlobBytes;
     if constexpr (!CH && !DUMP) { s1 += GS * kTileRows; s2 += GS * kTileRows; sq += GS * kTileRows; }
@@ -186,7 +207,13 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       if (ib0 < rb1) batch_setup();
     }
   };
-  for (int s = 0; s < kStages; ++s) issue_next();
+#pragma unroll
+  for (int s = 0; s < kStages; ++s) issue_next(false);  // weight side of the first stages
+  griddep_launch();                                     // the next kernel on the stream may start its own weight stream
+  griddep_wait();                                       // the quantizer's output is complete and visible from here on
+#pragma unroll
+  for (int s = 0; s < kStages; ++s)
+    if (s < n_pre) issue_tokens(my_stage0 + s * Cfg::kStageBytes, my_bar0 + 8 * s, aq_pre[s], sq_pre[s]);
 
   uint32_t par = 0;                                     // phase parity of the warp's stage barriers
   int cslot = 0;
@@ -337,7 +364,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
         }
       }
       __syncwarp();                                     // every lane is done reading the stage
-      issue_next();                                     // re-arm it with the warp's next k-block
+      issue_next(true);                                 // re-arm it with the warp's next k-block
       cslot = cslot + 1 == kStages ? 0 : cslot + 1;
     }
 
@@ -416,11 +443,11 @@ static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaS
   if (dump) {
     auto kern = w4a4_gemv_kernel<MT, true, CH, GS>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
-    kern<<<grid, kThreads, smem, st>>>(p);
+    if ((e = launch_pdl(kern, dim3(grid), dim3(kThreads), smem, st, p)) != cudaSuccess) return e;
   } else {
     auto kern = w4a4_gemv_kernel<MT, false, CH, GS>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
-    kern<<<grid, kThreads, smem, st>>>(p);
+    if ((e = launch_pdl(kern, dim3(grid), dim3(kThreads), smem, st, p)) != cudaSuccess) return e;
   }
   return cudaGetLastError();
 }

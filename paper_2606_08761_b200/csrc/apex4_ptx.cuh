@@ -19,6 +19,15 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
 #define APEX4_WATCHDOG_SPINS (1u << 26)
 #endif
 
+// ------------------------------------------------------------------ programmatic dependent launch
+// A kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start while its
+// predecessor on the stream is still running.  griddep_wait() blocks until the predecessor grid has
+// completed and its memory is visible: everything a kernel does before it must neither read what the
+// predecessor may have written nor write anything.  griddep_launch() lets the successor start its own
+// pre-wait part.  Both are no-ops in a plain launch.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ------------------------------------------------------------------ mbarrier
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));

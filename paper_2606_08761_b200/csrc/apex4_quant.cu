@@ -10,7 +10,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "apex4_gemm.cuh"
 #include "apex4_layout.cuh"
+#include "apex4_ptx.cuh"
 
 namespace apex4 {
 
@@ -117,6 +119,10 @@ __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __r
                                                                __half* __restrict__ S, int weights) {
   // 32-bit chunk index (the launcher checks R * K / 32 < 2^32): a 64-bit division here was ~150 of the
   // ~500 instructions of a thread
+  // programmatic dependent launch: X may come from the previous kernel on the stream (wait for it); the next
+  // kernel (the GEMM) may start streaming its weights while this one runs
+  griddep_wait();
+  if (!weights) griddep_launch();   // never ahead of a weight pack: the decode GEMM reads weights before its own wait
   const uint32_t cpr = static_cast<uint32_t>(K) / 32u;
   const uint32_t total = static_cast<uint32_t>(R) * cpr;
   uint32_t gid = blockIdx.x * 256u + threadIdx.x;
@@ -161,6 +167,8 @@ template <int U>   // chunks per thread (1, 2 or kLargeUnroll): fewer live regis
 __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
     const __half* __restrict__ X, int R, int K, int g, uint8_t* __restrict__ q,
     __half* __restrict__ S, int weights) {
+  griddep_wait();
+  if (!weights) griddep_launch();
   const int G = K / g;
   const int r = blockIdx.x / G;
   const int gamma = blockIdx.x % G;
@@ -293,26 +301,27 @@ cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s
   const long long total = static_cast<long long>(R) * (K / 32);
   const unsigned blocks = static_cast<unsigned>((total + 255) / 256);
   const bool pow2 = (gl & (gl - 1)) == 0;
+  cudaError_t e = cudaSuccess;
   if (pow2 && gl <= 32) {
     if (total + 256 > 0xFFFFFFFFll) return cudaErrorInvalidValue;   // 32-bit chunk index in the kernel
     switch (gl) {
-      case 1: quantize_small_g_kernel<1><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
-      case 2: quantize_small_g_kernel<2><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
-      case 4: quantize_small_g_kernel<4><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
-      case 8: quantize_small_g_kernel<8><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
-      case 16: quantize_small_g_kernel<16><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
-      default: quantize_small_g_kernel<32><<<blocks, 256, 0, st>>>(X, R, K, Q, S, weights); break;
+      case 1: e = launch_pdl(quantize_small_g_kernel<1>, dim3(blocks), dim3(256), 0, st, X, R, K, Q, S, weights); break;
+      case 2: e = launch_pdl(quantize_small_g_kernel<2>, dim3(blocks), dim3(256), 0, st, X, R, K, Q, S, weights); break;
+      case 4: e = launch_pdl(quantize_small_g_kernel<4>, dim3(blocks), dim3(256), 0, st, X, R, K, Q, S, weights); break;
+      case 8: e = launch_pdl(quantize_small_g_kernel<8>, dim3(blocks), dim3(256), 0, st, X, R, K, Q, S, weights); break;
+      case 16: e = launch_pdl(quantize_small_g_kernel<16>, dim3(blocks), dim3(256), 0, st, X, R, K, Q, S, weights); break;
+      default: e = launch_pdl(quantize_small_g_kernel<32>, dim3(blocks), dim3(256), 0, st, X, R, K, Q, S, weights); break;
     }
   } else {
     if (gl > kLargeThreads * kLargeUnroll) return cudaErrorInvalidValue;
     const long long nb = static_cast<long long>(R) * (K / g);
     const int threads = gl >= kLargeThreads ? kLargeThreads : (gl + 31) / 32 * 32;
     const unsigned nbu = static_cast<unsigned>(nb);
-    if (gl <= kLargeThreads) quantize_large_g_kernel<1><<<nbu, threads, 0, st>>>(X, R, K, g, Q, S, weights);
-    else if (gl <= 2 * kLargeThreads) quantize_large_g_kernel<2><<<nbu, threads, 0, st>>>(X, R, K, g, Q, S, weights);
-    else quantize_large_g_kernel<kLargeUnroll><<<nbu, threads, 0, st>>>(X, R, K, g, Q, S, weights);
+    if (gl <= kLargeThreads) e = launch_pdl(quantize_large_g_kernel<1>, dim3(nbu), dim3(threads), 0, st, X, R, K, g, Q, S, weights);
+    else if (gl <= 2 * kLargeThreads) e = launch_pdl(quantize_large_g_kernel<2>, dim3(nbu), dim3(threads), 0, st, X, R, K, g, Q, S, weights);
+    else e = launch_pdl(quantize_large_g_kernel<kLargeUnroll>, dim3(nbu), dim3(threads), 0, st, X, R, K, g, Q, S, weights);
   }
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 bool quantize_supports_group(int g) {
   const int gl = g / 32;

@@ -22,6 +22,8 @@ def read_kv_fixture(name):
             line = line.strip()
             if not line or line.startswith("#"):
                 continue
+            if "=" not in line:
+                continue              # a row of a mixed fixture (read_rows_fixture reads those)
             k, v = line.split("=", 1)
             out[k.strip()] = v.split()
     return out

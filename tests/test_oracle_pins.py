@@ -385,3 +385,119 @@ def test_pin_f32_ordered_sum():
                 s = Fraction(float(r["sA"][m, gam])) * Fraction(float(r["sW"][n, gam]))     # 22 bits: exact in binary32
                 acc = _rn_f32(P * s + acc)
             assert Fraction(float(Y32[m, n])) == acc, (m, n)
+
+
+# ----------------------------------------------------------------- P9: producers of the quantizer's input
+def test_p9_silu_mul_hand_values_and_invariants():
+    rows = [r for r in read_rows_fixture("p9_producers.txt") if r[0] == "silu"]
+    assert len(rows) >= 8
+    for _, g, u, want in rows:
+        y = O.silu_mul(f16([g])[None, :], f16([u])[None, :])
+        assert int(bits(y)[0, 0]) == int(want, 16), (g, u, hex(int(bits(y)[0, 0])))
+    rng = np.random.default_rng(21)
+    g = (rng.standard_normal((7, 96)) * 4).astype(np.float16)
+    u = rng.standard_normal((7, 96)).astype(np.float16)
+    y = O.silu_mul(g, u).astype(np.float64)
+    # silu(g) - silu(-g) = g, silu(g) in (min(g,0) - 0.2785, max(g, 0)), sign(y) = sign(g) sign(u), odd in up
+    g64, u64 = g.astype(np.float64), u.astype(np.float64)
+    s = g64 / (1 + np.exp(-g64))
+    assert np.allclose(s - (-g64) / (1 + np.exp(g64)), g64, rtol=0, atol=1e-12)
+    assert np.all(np.abs(y - s * u64) <= np.maximum(np.abs(s * u64) * 2.0 ** -11, 2.0 ** -25))     # half an FP16 ulp
+    assert np.array_equal(O.silu_mul(g, (-u).astype(np.float16)).view(np.uint16) ^ 0x8000, O.silu_mul(g, u).view(np.uint16))
+
+
+def test_p9_silu_every_fp16_gate_against_50_digit_decimal():
+    """Independent restatement: silu(g) with 50-digit decimal arithmetic, rounded once to FP16 with integer
+    arithmetic (ties to even), for EVERY finite FP16 gate and up = 1, and for a second up on a subset."""
+    from decimal import Decimal, getcontext
+    from fractions import Fraction
+    getcontext().prec = 50
+
+    def rn_f16_bits(x: Fraction) -> int:
+        if x == 0:
+            return 0
+        sgn = 0x8000 if x < 0 else 0
+        x = abs(x)
+        e = 0
+        while x >= 2048:
+            x /= 2; e += 1
+        while x < 1024 and e > -24:          # 11-bit significand, subnormals stop at 2^-24 units
+            x *= 2; e -= 1
+        n, rem = divmod(x.numerator, x.denominator)
+        if 2 * rem > x.denominator or (2 * rem == x.denominator and n % 2 == 1):
+            n += 1
+        if n == 2048:
+            n = 1024; e += 1
+        val = Fraction(n) * Fraction(2) ** e
+        return sgn | int(np.array([float(val)], dtype=np.float64).astype(np.float16).view(np.uint16)[0])   # exact: val is an FP16 value
+
+    allb = np.arange(0x10000, dtype=np.uint32).astype(np.uint16)
+    finite = allb[((allb >> 10) & 0x1F) != 0x1F]
+    gates = finite.view(np.float16)
+    got = O.silu_mul(gates[None, :], np.ones((1, gates.size), dtype=np.float16)).view(np.uint16)[0]
+    step = 1           # every gate
+    bad = 0
+    for idx in range(0, gates.size, step):
+        gd = Decimal(float(gates[idx]))
+        if gd == 0:
+            want = 0x8000 if (finite[idx] & 0x8000) else 0      # silu(-0) * 1 = -0 / 2 = -0
+        else:
+            if gd < -120:                        # e^-g overflows nothing in decimal, but keep it cheap: silu -> -|g| e^g ~ 0-
+                sd = gd * (gd.exp())             # g / (1 + e^-g) = g e^g / (e^g + 1); e^g + 1 = 1 to 50 digits
+            else:
+                sd = gd / (1 + (-gd).exp())
+            want = rn_f16_bits(Fraction(sd))
+            if want & 0x7FFF == 0:
+                want = 0x8000 if gd < 0 else 0
+        if int(got[idx]) != want:
+            bad += 1
+            assert bad < 1, (hex(int(finite[idx])), hex(int(got[idx])), hex(want))
+    assert bad == 0
+
+
+def test_p9_rmsnorm_hand_values_invariants_and_exact_restatement():
+    from fractions import Fraction
+    import math
+    fx = read_kv_fixture("p9_producers.txt")
+    x = f16(fx["rmsnorm_x"])[None, :]
+    y = O.rmsnorm(x, np.ones(4, dtype=np.float16), 0.0)
+    assert [int(b) for b in bits(y)[0]] == [int(v, 16) for v in fx["rmsnorm_gamma1"]]
+    y = O.rmsnorm(x, f16(fx["rmsnorm_gamma2_in"]), 0.0)
+    assert [int(b) for b in bits(y)[0]] == [int(v, 16) for v in fx["rmsnorm_gamma2"]]
+    # constant rows with power-of-two magnitude normalise to exactly +-1; scaling x by 2^j changes nothing (eps = 0)
+    assert np.all(O.rmsnorm(np.full((2, 64), 4.0, dtype=np.float16), np.ones(64, dtype=np.float16), 0.0) == 1.0)
+    rng = np.random.default_rng(22)
+    X = rng.standard_normal((5, 256)).astype(np.float16)
+    gam = (1 + 0.1 * rng.standard_normal(256)).astype(np.float16)
+    base = O.rmsnorm(X, gam, 0.0)
+    assert np.array_equal(O.rmsnorm((X.astype(np.float32) * 8).astype(np.float16), gam, 0.0).view(np.uint16), base.view(np.uint16))
+    assert np.array_equal(O.rmsnorm(-X, gam, 0.0).view(np.uint16), base.view(np.uint16) ^ 0x8000)
+    # against the real-valued definition x gamma / sqrt(mean(x^2) + eps): three binary32 roundings + one FP16 rounding
+    eps = 1e-5
+    y = O.rmsnorm(X, gam, eps).astype(np.float64)
+    X64 = X.astype(np.float64)
+    ref = X64 * gam.astype(np.float64)[None, :] / np.sqrt(np.mean(X64 * X64, axis=1, keepdims=True) + eps)
+    assert np.all(np.abs(y - ref) <= np.abs(ref) * (2.0 ** -11 + 4 * 2.0 ** -24) + 2.0 ** -25)
+    # exact-rational restatement of the binary32 sequence (own rn32, integer square root) on a small case
+    def rn32_sqrt(q: Fraction) -> Fraction:
+        # correctly rounded binary32 square root of a positive rational: integer sqrt at 2^-60 relative, then rn32
+        sc = 0
+        while q * Fraction(4) ** sc < Fraction(2) ** 120:
+            sc += 1
+        v = q * Fraction(4) ** sc
+        r = math.isqrt(v.numerator // v.denominator)
+        cand = Fraction(r, 2 ** sc)
+        lo, hi = _rn_f32(cand), _rn_f32(Fraction(r + 1, 2 ** sc))
+        assert lo == hi                      # not within 2^-60 of a rounding boundary
+        return lo
+    Xs = X[:2, :32]
+    gs = gam[:32]
+    ys = O.rmsnorm(Xs, gs, eps)
+    eps32 = Fraction(float(np.float32(eps)))
+    for m in range(2):
+        ss = sum(Fraction(float(v)) ** 2 for v in Xs[m])
+        ms = _rn_f32(ss / 32)
+        inv = _rn_f32(1 / rn32_sqrt(_rn_f32(ms + eps32)))
+        for k in range(32):
+            y32 = _rn_f32(_rn_f32(Fraction(float(Xs[m, k])) * inv) * Fraction(float(gs[k])))
+            assert float(ys[m, k]) == float(np.float16(float(y32))), (m, k)      # float(y32) is exact; one FP16 rounding
