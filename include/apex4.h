@@ -123,6 +123,20 @@ const char* apex4_status_string(int status);
 int apex4_quantize_act(const void* x_f16, int M, int K, int group_size, int gran, int layer,
                        void* qA_packed, void* sA_f16, void* stream);
 
+/* ---- a1 fused into its producer ("quantized online") ------------------------- */
+/* The two ops that feed the linears of a Llama / Qwen block, with the quantizer of Eq. 7 applied to their FP16
+ * result before it ever reaches HBM.  Outputs are exactly apex4_quantize_act of that FP16 result (same layouts,
+ * same sizes); y_f16_out, if not NULL, also receives the FP16 result [M,K] (verification, residual paths).
+ *   apex4_rmsnorm_quantize:  y = fp16( (x * inv) * gamma ),  inv = 1.0f / sqrtf( float(sum_k x^2 / K) + eps ),
+ *       the sum of squares exact, every other step one IEEE binary32 operation (R17).  gamma_f16 [K].
+ *   apex4_silu_mul_quantize: y = fp16( silu(gate) * up ), silu(g) = g / (1 + exp(-g)), the real-valued product
+ *       rounded once (R18).  gate_f16 / up_f16 [M,K] with row stride ld >= K elements (ld % 8 == 0), so
+ *       the two halves of a fused gate+up GEMM output [M, 2K] can be passed as (Y, Y + K, ld = 2K). */
+int apex4_rmsnorm_quantize(const void* x_f16, const void* gamma_f16, float eps, int M, int K, int group_size,
+                           int gran, int layer, void* qA_packed, void* sA_f16, void* y_f16_out, void* stream);
+int apex4_silu_mul_quantize(const void* gate_f16, const void* up_f16, int ld, int M, int K, int group_size,
+                            int gran, int layer, void* qA_packed, void* sA_f16, void* y_f16_out, void* stream);
+
 /* ---- a0: offline weight quantize + pack (Eq. 7) --------------------------- */
 /* w_f16 [N,K] FP16 -> qW_packed (PW4) + sW_f16 (ST16). Same arithmetic as the activation quantizer. */
 int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran, int layer,

@@ -27,6 +27,7 @@ OPERAND_ACT, OPERAND_WEIGHT = 0, 1
 EXPORTS = (
     "apex4_resolve_group_size", "apex4_packed_bytes", "apex4_scale_elems", "apex4_workspace_bytes",
     "apex4_workspace_bytes_ex", "apex4_status_string", "apex4_quantize_act", "apex4_pack_weights",
+    "apex4_rmsnorm_quantize", "apex4_silu_mul_quantize",
     "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
     "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes",
     "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho",
@@ -87,6 +88,12 @@ def lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
         f.restype = c_int
+    L.apex4_rmsnorm_quantize.argtypes = [c_void_p, c_void_p, ctypes.c_float, c_int, c_int, c_int, c_int, c_int, c_void_p, c_void_p,
+                                         c_void_p, c_void_p]
+    L.apex4_silu_mul_quantize.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_int, c_int, c_void_p, c_void_p,
+                                          c_void_p, c_void_p]
+    L.apex4_rmsnorm_quantize.restype = c_int
+    L.apex4_silu_mul_quantize.restype = c_int
     L.apex4_pack_codes.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
     L.apex4_unpack_codes.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
     L.apex4_scales_from_natural.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p]
@@ -174,6 +181,45 @@ def quantize_act(x, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, q=None, 
 def pack_weights(w, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, q=None, s=None):
     """apex4_pack_weights: W[N,K] fp16 -> (qW PW4, sW ST16, g)."""
     return _quantize("apex4_pack_weights", w, group_size, gran, layer, q, s)
+
+
+def _fused_out(M, K, g, device, q, s, want_y):
+    if q is None:
+        q = torch.empty(packed_bytes(M, K), dtype=torch.uint8, device=device)
+    if s is None:
+        s = torch.empty(scale_elems(M, K, g), dtype=torch.float16, device=device)
+    y = torch.empty((M, K), dtype=torch.float16, device=device) if want_y else None
+    return q, s, y
+
+
+def rmsnorm_quantize(x, gamma, eps: float, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, q=None, s=None, want_y=False):
+    """apex4_rmsnorm_quantize: X[M,K], gamma[K] fp16 -> (qA PT4, sA ST16, g[, y fp16 [M,K]])."""
+    _dev(x, torch.float16, "apex4_rmsnorm_quantize")
+    _dev(gamma, torch.float16, "apex4_rmsnorm_quantize")
+    M, K = x.shape
+    g = resolve_group_size(K, group_size, gran, layer)
+    q, s, y = _fused_out(M, K, g, x.device, q, s, want_y)
+    st = lib().apex4_rmsnorm_quantize(x.data_ptr(), gamma.data_ptr(), float(eps), M, K, group_size, gran, layer, q.data_ptr(),
+                                      s.data_ptr(), y.data_ptr() if y is not None else None, _stream())
+    _check(st, "apex4_rmsnorm_quantize")
+    return (q, s, g, y) if want_y else (q, s, g)
+
+
+def silu_mul_quantize(gate, up, group_size=128, gran=GRAN_GROUP, layer=LAYER_OTHER, q=None, s=None, want_y=False):
+    """apex4_silu_mul_quantize: gate, up [M,K] fp16 (views of one [M, 2K] tensor allowed: row stride >= K)
+    -> (qA PT4, sA ST16, g[, y fp16 [M,K]])."""
+    for t in (gate, up):
+        if not t.is_cuda or t.dtype != torch.float16 or t.dim() != 2 or t.stride(1) != 1:
+            raise ValueError("apex4_silu_mul_quantize: expected 2-D CUDA float16 tensors with unit column stride")
+    if gate.shape != up.shape or gate.stride(0) != up.stride(0):
+        raise ValueError("apex4_silu_mul_quantize: gate and up must have the same shape and row stride")
+    M, K = gate.shape
+    g = resolve_group_size(K, group_size, gran, layer)
+    q, s, y = _fused_out(M, K, g, gate.device, q, s, want_y)
+    st = lib().apex4_silu_mul_quantize(gate.data_ptr(), up.data_ptr(), gate.stride(0), M, K, group_size, gran, layer, q.data_ptr(),
+                                       s.data_ptr(), y.data_ptr() if y is not None else None, _stream())
+    _check(st, "apex4_silu_mul_quantize")
+    return (q, s, g, y) if want_y else (q, s, g)
 
 
 def pack_codes(codes: torch.Tensor, operand: int) -> torch.Tensor:

@@ -14,6 +14,10 @@ namespace apex4 {
 cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, int weights,
                             cudaStream_t st);
 bool quantize_supports_group(int g);
+cudaError_t launch_rmsnorm_quantize(const void* x, const void* gamma, float eps, int R, int K, int g, void* q, void* s, void* y_out,
+                                    cudaStream_t st);
+cudaError_t launch_silu_mul_quantize(const void* gate, const void* up, int ld, int R, int K, int g, void* q, void* s, void* y_out,
+                                     cudaStream_t st);
 cudaError_t launch_pack_codes(const int8_t* codes, int R, int K, void* q, int weights, cudaStream_t st);
 cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, int weights, cudaStream_t st);
 cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st);
@@ -232,6 +236,39 @@ int apex4_quantize_act(const void* x_f16, int M, int K, int group_size, int gran
 int apex4_pack_weights(const void* w_f16, int N, int K, int group_size, int gran, int layer,
                        void* qW_packed, void* sW_f16, void* stream) {
   return quantize_common(w_f16, N, K, group_size, gran, layer, qW_packed, sW_f16, 1, stream);
+}
+
+int apex4_rmsnorm_quantize(const void* x_f16, const void* gamma_f16, float eps, int M, int K, int group_size, int gran,
+                           int layer, void* qA_packed, void* sA_f16, void* y_f16_out, void* stream) {
+  if (!x_f16 || !gamma_f16 || !qA_packed || !sA_f16 || M < 1 || K < 1 || !(eps >= 0.f)) return APEX4_ERR_INVALID_ARG;
+  if (K > 32768) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  if (!aligned16(x_f16) || !aligned16(gamma_f16) || !aligned16(qA_packed) || !aligned16(sA_f16) || !aligned16(y_f16_out))
+    return APEX4_ERR_ALIGNMENT;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_rmsnorm_quantize(x_f16, gamma_f16, eps, M, K, g, qA_packed, sA_f16, y_f16_out, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
+}
+
+int apex4_silu_mul_quantize(const void* gate_f16, const void* up_f16, int ld, int M, int K, int group_size, int gran, int layer,
+                            void* qA_packed, void* sA_f16, void* y_f16_out, void* stream) {
+  if (!gate_f16 || !up_f16 || !qA_packed || !sA_f16 || M < 1 || K < 1 || ld < K) return APEX4_ERR_INVALID_ARG;
+  if (K > 32768) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  const int g = resolve_g(K, group_size, gran, layer);
+  if (g < 0) return -g;
+  if (!aligned16(gate_f16) || !aligned16(up_f16) || (ld % 8) != 0 || !aligned16(qA_packed) || !aligned16(sA_f16) ||
+      !aligned16(y_f16_out))
+    return APEX4_ERR_ALIGNMENT;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return launch_silu_mul_quantize(gate_f16, up_f16, ld, M, K, g, qA_packed, sA_f16, y_f16_out, static_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess
+             ? APEX4_OK
+             : APEX4_ERR_CUDA;
 }
 
 int apex4_pack_codes(const int8_t* codes, int R, int K, int operand, void* q_packed, void* stream) {

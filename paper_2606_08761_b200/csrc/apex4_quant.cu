@@ -20,8 +20,8 @@ namespace apex4 {
 // One thread = one 32-element chunk; a group is GL = g/32 consecutive lanes of a warp (GL in 1..32).
 // Rows R .. roundup(R, 128) - 1 (the padding of the last 128-row blob, which the GEMM kernels bulk-copy and
 // consume) are written as zero codes and zero scales.
-template <int GL>
-__global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __restrict__ X, int R, int Rp,
+template <int GL, class Producer>
+__global__ void __launch_bounds__(256) quantize_small_g_kernel(const Producer prod, int R, int Rp,
                                                                int K, uint8_t* __restrict__ q,
                                                                __half* __restrict__ S, int weights) {
   // programmatic dependent launch: X may come from the previous kernel on the stream (wait for it); the next
@@ -37,13 +37,8 @@ __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __r
   const int r = static_cast<int>(gid / cpr);
   const int c = static_cast<int>(gid - static_cast<uint32_t>(r) * cpr);
   uint32_t w[16];
-  if (r < R) {
-    const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + c * 32);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const uint4 v = __ldg(src + i);
-      w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
-    }
+  if (r < R && active) {
+    prod.load(r, c, w);
   } else {
 #pragma unroll
     for (int i = 0; i < 16; ++i) w[i] = 0u;
@@ -65,9 +60,9 @@ __global__ void __launch_bounds__(256) quantize_small_g_kernel(const __half* __r
 // the absmax pass and the quantize pass.
 constexpr int kLargeThreads = 256;
 constexpr int kLargeUnroll = 4;
-template <int U>   // chunks per thread (1, 2 or kLargeUnroll): fewer live registers, more blocks per SM
+template <int U, class Producer>   // U chunks per thread (1, 2 or kLargeUnroll): fewer live registers, more blocks per SM
 __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
-    const __half* __restrict__ X, int R, int K, int g, uint8_t* __restrict__ q,
+    const Producer prod, int R, int K, int g, uint8_t* __restrict__ q,
     __half* __restrict__ S, int weights) {
   griddep_wait();
   if (!weights) griddep_launch();
@@ -84,12 +79,7 @@ __global__ void __launch_bounds__(kLargeThreads) quantize_large_g_kernel(
   for (int u = 0; u < U; ++u) {
     const int cl = threadIdx.x + u * nthr;
     if (cl < cpg && r < R) {
-      const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + (c0 + cl) * 32);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const uint4 v = __ldg(src + i);
-        w[u][4 * i] = v.x; w[u][4 * i + 1] = v.y; w[u][4 * i + 2] = v.z; w[u][4 * i + 3] = v.w;
-      }
+      prod.load(r, c0 + cl, w[u]);
       m = absmax_bits_max(m, chunk_absmax_bits(w[u]));
     } else {
 #pragma unroll
@@ -188,9 +178,8 @@ __global__ void scales_to_natural_kernel(const __half* __restrict__ tiled, int R
 }
 
 // ---------------------------------------------------------------------------------- launchers
-cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, int weights,
-                            cudaStream_t st) {
-  const __half* X = static_cast<const __half*>(x);
+template <class Producer>
+static cudaError_t launch_quantize_with(const Producer& prod, int R, int K, int g, void* q, void* s, int weights, cudaStream_t st) {
   uint8_t* Q = static_cast<uint8_t*>(q);
   __half* S = static_cast<__half*>(s);
   const int gl = g / 32;
@@ -202,24 +191,36 @@ cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s
   if (pow2 && gl <= 32) {
     if (total + 256 > 0xFFFFFFFFll) return cudaErrorInvalidValue;   // 32-bit chunk index in the kernel
     switch (gl) {
-      case 1: e = launch_pdl(quantize_small_g_kernel<1>, dim3(blocks), dim3(256), 0, st, X, R, Rp, K, Q, S, weights); break;
-      case 2: e = launch_pdl(quantize_small_g_kernel<2>, dim3(blocks), dim3(256), 0, st, X, R, Rp, K, Q, S, weights); break;
-      case 4: e = launch_pdl(quantize_small_g_kernel<4>, dim3(blocks), dim3(256), 0, st, X, R, Rp, K, Q, S, weights); break;
-      case 8: e = launch_pdl(quantize_small_g_kernel<8>, dim3(blocks), dim3(256), 0, st, X, R, Rp, K, Q, S, weights); break;
-      case 16: e = launch_pdl(quantize_small_g_kernel<16>, dim3(blocks), dim3(256), 0, st, X, R, Rp, K, Q, S, weights); break;
-      default: e = launch_pdl(quantize_small_g_kernel<32>, dim3(blocks), dim3(256), 0, st, X, R, Rp, K, Q, S, weights); break;
+      case 1: e = launch_pdl(quantize_small_g_kernel<1, Producer>, dim3(blocks), dim3(256), 0, st, prod, R, Rp, K, Q, S, weights); break;
+      case 2: e = launch_pdl(quantize_small_g_kernel<2, Producer>, dim3(blocks), dim3(256), 0, st, prod, R, Rp, K, Q, S, weights); break;
+      case 4: e = launch_pdl(quantize_small_g_kernel<4, Producer>, dim3(blocks), dim3(256), 0, st, prod, R, Rp, K, Q, S, weights); break;
+      case 8: e = launch_pdl(quantize_small_g_kernel<8, Producer>, dim3(blocks), dim3(256), 0, st, prod, R, Rp, K, Q, S, weights); break;
+      case 16: e = launch_pdl(quantize_small_g_kernel<16, Producer>, dim3(blocks), dim3(256), 0, st, prod, R, Rp, K, Q, S, weights); break;
+      default: e = launch_pdl(quantize_small_g_kernel<32, Producer>, dim3(blocks), dim3(256), 0, st, prod, R, Rp, K, Q, S, weights); break;
     }
   } else {
     if (gl > kLargeThreads * kLargeUnroll) return cudaErrorInvalidValue;
     const long long nb = static_cast<long long>(Rp) * (K / g);
     const int threads = gl >= kLargeThreads ? kLargeThreads : (gl + 31) / 32 * 32;
     const unsigned nbu = static_cast<unsigned>(nb);
-    if (gl <= kLargeThreads) e = launch_pdl(quantize_large_g_kernel<1>, dim3(nbu), dim3(threads), 0, st, X, R, K, g, Q, S, weights);
-    else if (gl <= 2 * kLargeThreads) e = launch_pdl(quantize_large_g_kernel<2>, dim3(nbu), dim3(threads), 0, st, X, R, K, g, Q, S, weights);
-    else e = launch_pdl(quantize_large_g_kernel<kLargeUnroll>, dim3(nbu), dim3(threads), 0, st, X, R, K, g, Q, S, weights);
+    if (gl <= kLargeThreads) e = launch_pdl(quantize_large_g_kernel<1, Producer>, dim3(nbu), dim3(threads), 0, st, prod, R, K, g, Q, S, weights);
+    else if (gl <= 2 * kLargeThreads) e = launch_pdl(quantize_large_g_kernel<2, Producer>, dim3(nbu), dim3(threads), 0, st, prod, R, K, g, Q, S, weights);
+    else e = launch_pdl(quantize_large_g_kernel<kLargeUnroll, Producer>, dim3(nbu), dim3(threads), 0, st, prod, R, K, g, Q, S, weights);
   }
   return e != cudaSuccess ? e : cudaGetLastError();
 }
+
+cudaError_t launch_quantize(const void* x, int R, int K, int g, void* q, void* s, int weights, cudaStream_t st) {
+  return launch_quantize_with(PlainLoad{static_cast<const __half*>(x), K}, R, K, g, q, s, weights, st);
+}
+
+// SiLU(gate) * up fused into the quantizer: the same kernels with another producer of the chunk
+cudaError_t launch_silu_mul_quantize(const void* gate, const void* up, int ld, int R, int K, int g, void* q, void* s, void* y_out,
+                                     cudaStream_t st) {
+  return launch_quantize_with(SiluMulLoad{static_cast<const __half*>(gate), static_cast<const __half*>(up), static_cast<__half*>(y_out), ld, K},
+                              R, K, g, q, s, 0, st);
+}
+
 bool quantize_supports_group(int g) {
   const int gl = g / 32;
   return ((gl & (gl - 1)) == 0 && gl <= 32) || gl <= kLargeThreads * kLargeUnroll;

@@ -99,6 +99,78 @@ __device__ __forceinline__ uint4 quant_chunk(const uint32_t (&w)[16], float s) {
   return make_uint4(out[0], out[1], out[2], out[3]);
 }
 
+// ------------------------------------------------------------------ producers of a chunk (what the quantizer kernels read)
+// plain: the FP16 activation / weight matrix itself
+struct PlainLoad {
+  const __half* X;
+  int K;
+  __device__ __forceinline__ void load(int r, int c, uint32_t (&w)[16]) const {
+    const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(r) * K + c * 32);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const uint4 v = __ldg(src + i);
+      w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
+    }
+  }
+};
+
+// y = fp16(silu(g) * u), silu(g) = g / (1 + exp(-g)): the real-valued product rounded ONCE (R18).
+// Fast path in binary32 with relative error below 1.25 * 2^-21 = 10 * 2^-24:
+//   exp(-g) = ex2(th) * (1 + tl ln 2), th + tl = -g log2(e) to ~2^-45 (th = fl(-g L1), tl its FMA residual plus -g L2):
+//             ex2.approx <= 2^-22 relative (PTX ISA), the correction factor adds 2^-24;
+//   1 + e: 2^-24;  rcp.approx: 2^-23 (PTX ISA);  g * r and * u: 2^-24 each.
+// The result is accepted when both ends of a +-2^-20 interval round to the same FP16 value (rounding is monotonic);
+// otherwise (~0.3 % of the elements: an FP16 rounding boundary inside the interval), and for |g| > 83 where ex2 leaves
+// its normal range, it is recomputed in binary64.
+__device__ __forceinline__ __half silu_mul_one(float g, float u) {
+  const float L1 = 1.44269502162933349609375f;          // fl(log2 e)
+  const float L2 = 1.9259629911783013e-08f;             // log2 e - L1
+  const float th = __fmul_rn(-g, L1);
+  const float tl = __fmaf_rn(-g, L2, __fmaf_rn(-g, L1, -th));
+  float e;
+  asm("ex2.approx.f32 %0, %1;" : "=f"(e) : "f"(th));
+  e = __fmul_rn(e, __fmaf_rn(tl, 0.693147182464599609375f, 1.0f));
+  const float d = __fadd_rn(1.0f, e);
+  float r;
+  asm("rcp.approx.f32 %0, %1;" : "=f"(r) : "f"(d));
+  const float y = __fmul_rn(__fmul_rn(g, r), u);
+  const __half lo = __float2half_rn(y * 0.99999904632568359375f);   // 1 - 2^-20
+  const __half hi = __float2half_rn(y * 1.00000095367431640625f);   // 1 + 2^-20
+  // th in the normal range of ex2 and 1 + e finite: otherwise (g < -87: e overflows; g > 87: e is flushed) take the slow path
+  if (__half_as_ushort(lo) == __half_as_ushort(hi) && fabsf(th) < 120.0f) return lo;
+  const double gd = static_cast<double>(g);
+  const double s = gd / (1.0 + exp(-gd));               // exp(-gd) = inf for gd < -709: s = -0, as in the oracle
+  return __double2half(s * static_cast<double>(u));
+}
+
+struct SiluMulLoad {
+  const __half* gate;
+  const __half* up;
+  __half* y_out;                                        // optional FP16 copy [M,K]
+  int ld, K;
+  __device__ __forceinline__ void load(int r, int c, uint32_t (&w)[16]) const {
+    const uint4* gsrc = reinterpret_cast<const uint4*>(gate + static_cast<size_t>(r) * ld + c * 32);
+    const uint4* usrc = reinterpret_cast<const uint4*>(up + static_cast<size_t>(r) * ld + c * 32);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const uint4 gv = __ldg(gsrc + i), uv = __ldg(usrc + i);
+      const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w}, uw[4] = {uv.x, uv.y, uv.z, uv.w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float2 gf = __half22float2(*reinterpret_cast<const __half2*>(&gw[j]));
+        const float2 uf = __half22float2(*reinterpret_cast<const __half2*>(&uw[j]));
+        const __half2 y = __halves2half2(silu_mul_one(gf.x, uf.x), silu_mul_one(gf.y, uf.y));
+        w[4 * i + j] = *reinterpret_cast<const uint32_t*>(&y);
+      }
+    }
+    if (y_out != nullptr) {
+      uint4* dst = reinterpret_cast<uint4*>(y_out + static_cast<size_t>(r) * K + c * 32);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) dst[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+    }
+  }
+};
+
 // PT4 odd rows keep the second 16-element half in the LOW nibbles (apex4_layout.cuh): exchange the nibbles of every byte
 __device__ __forceinline__ uint4 nibble_swap(uint4 v) {
   auto sw = [](uint32_t x) { return ((x >> 4) & 0x0F0F0F0Fu) | ((x << 4) & 0xF0F0F0F0u); };
