@@ -203,6 +203,16 @@ int apex4_debug_get_dispatch(int M, int N, int K, int group_size, int gran, int 
  * does). */
 int apex4_measure_rho(double* out_host, void* stream);
 
+/* ---- experiment: is an FP8 tensor-core path exact on INT4 codes? ------------------------------- */
+/* Runs one 128 x 256 tile over K (multiple of 128, <= 32768) through tcgen05.mma kind::i8 and through
+ * kind::f8f6f4 with the same codes as E4M3 operands and compares the two TMEM accumulators element by element.
+ * pattern: 0 uniform codes, 1 all -8, 2 alternating 7 / -8, 3 large sums with odd increments, 4 random signs at
+ * +-7, 5 deterministic ramp.  encoding: 0 = codes as normal E4M3 numbers, 1 = sign | magnitude (E4M3 subnormals,
+ * value code * 2^-9).  out_host (HOST, >= 5 doubles) = {mismatching elements, max |fp32 - int|, max |int sum|,
+ * elements compared, mismatches of the INT8 sums against 64 K (pattern 1 only)}.  Synchronises the stream and
+ * allocates / frees 40 bytes of device scratch.  Not a product path: apex4_w4a4_gemm always uses kind::i8. */
+int apex4_e4m3_exactness(int K, int pattern, int encoding, unsigned seed, double* out_host, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

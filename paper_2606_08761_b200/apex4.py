@@ -30,7 +30,7 @@ EXPORTS = (
     "apex4_rmsnorm_quantize", "apex4_silu_mul_quantize",
     "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
     "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes",
-    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho",
+    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_e4m3_exactness",
 )
 
 
@@ -108,6 +108,8 @@ def lib() -> ctypes.CDLL:
     L.apex4_debug_group_sums.argtypes = [c_void_p, c_void_p] + [c_int] * 10 + [c_void_p, c_void_p,
                                                                               ctypes.POINTER(DebugOpts)]
     L.apex4_measure_rho.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
+    L.apex4_e4m3_exactness.argtypes = [c_int, c_int, c_int, ctypes.c_uint, ctypes.POINTER(ctypes.c_double), c_void_p]
+    L.apex4_e4m3_exactness.restype = c_int
     L.apex4_debug_get_dispatch.argtypes = [c_int] * 6 + [ctypes.POINTER(DebugOpts), ctypes.POINTER(c_int)]
     for name in ("apex4_pack_codes", "apex4_unpack_codes", "apex4_scales_from_natural",
                  "apex4_scales_to_natural", "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host",
@@ -321,6 +323,14 @@ def measure_rho() -> dict:
     _check(lib().apex4_measure_rho(out, _stream()), "apex4_measure_rho")
     keys = ("int8_tops", "fp32_tflops", "i2f_gops", "rho", "tmem_ld_gbs", "sm_clock_mhz",
             "int8_mac_per_clk_sm", "tmem_ld_bytes_per_clk_sm")
+    return dict(zip(keys, [float(v) for v in out]))
+
+
+def e4m3_exactness(K: int, pattern: int, encoding: int, seed: int = 0) -> dict:
+    """apex4_e4m3_exactness: kind::f8f6f4 (E4M3 operands, FP32 accumulate) against kind::i8 on the same INT4 codes."""
+    out = (ctypes.c_double * 5)()
+    _check(lib().apex4_e4m3_exactness(K, pattern, encoding, seed, out, _stream()), "apex4_e4m3_exactness")
+    keys = ("mismatches", "max_abs_diff", "max_abs_sum", "compared", "int8_vs_closed_form_mismatches")
     return dict(zip(keys, [float(v) for v in out]))
 
 

@@ -23,6 +23,7 @@ cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, int 
 cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st);
 cudaError_t launch_scales_to_natural(const void* tiled, int R, int G, void* nat, cudaStream_t st);
 int measure_rho(double* out, cudaStream_t st);
+int e4m3_exactness(int K, int pattern, int encoding, uint32_t seed, double* out, cudaStream_t st);
 }  // namespace apex4
 
 using namespace apex4;
@@ -443,6 +444,14 @@ int apex4_debug_get_dispatch(int M, int N, int K, int group_size, int gran, int 
   if (!choose_dispatch(M, N, K, g, opts ? *opts : kAuto, d)) return APEX4_ERR_INVALID_ARG;
   out5[0] = d.kernel; out5[1] = d.kernel == 1 ? d.pnt : 16 * d.mt; out5[2] = d.split; out5[3] = d.grid; out5[4] = d.upt;
   return APEX4_OK;
+}
+
+int apex4_e4m3_exactness(int K, int pattern, int encoding, unsigned seed, double* out_host, void* stream) {
+  if (!out_host || pattern < 0 || pattern > 5 || (encoding != 0 && encoding != 1)) return APEX4_ERR_INVALID_ARG;
+  if (K < kBlockK || K % kBlockK != 0 || K > 32768) return APEX4_ERR_UNSUPPORTED_SHAPE;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return e4m3_exactness(K, pattern, encoding, seed, out_host, static_cast<cudaStream_t>(stream));
 }
 
 int apex4_measure_rho(double* out_host, void* stream) {

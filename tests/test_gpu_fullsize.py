@@ -207,3 +207,19 @@ def test_rho_microbenchmark_ranges(A):
     assert 50 <= r["rho"] <= 70, r
     assert abs(r["rho"] - r["int8_tops"] / r["fp32_tflops"]) < 1e-6 * r["rho"]
     assert 150 <= r["tmem_ld_bytes_per_clk_sm"] <= 1100, r
+
+
+@pytest.mark.parametrize("encoding", [0, 1])
+def test_e4m3_tensor_path_is_exact_on_int4_codes(A, encoding):
+    """SURVEY 8(f)4 experiment (measured fact on B200, recorded in DESIGN.md): tcgen05.mma kind::f8f6f4 with the
+    codes as E4M3 operands and FP32 accumulation reproduces the kind::i8 sums exactly, up to per-channel K = 32768
+    (sums up to 2^21), for random, extreme, cancelling and odd-increment inputs; and the kind::i8 sums of the all-(-8)
+    pattern equal the closed form 64 K."""
+    for pattern in range(6):
+        for K in (128, 4096, 32768):
+            r = A.e4m3_exactness(K, pattern, encoding, seed=11 + pattern)
+            assert r["compared"] == 128 * 256
+            assert r["int8_vs_closed_form_mismatches"] == 0
+            assert r["mismatches"] == 0 and r["max_abs_diff"] == 0.0, (pattern, K, r)
+            if pattern == 1:
+                assert r["max_abs_sum"] == 64 * K
