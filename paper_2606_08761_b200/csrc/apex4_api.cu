@@ -89,11 +89,12 @@ int pair_tokens(int M, const apex4_debug_opts& o) {
   return 6 * r128 < 5 * r192 ? 128 : kPairTokens;
 }
 
-// The decode kernel covers M <= 32 at g = 32 / 64 / 128 and per-channel (groups in between need one
-// rounding per group, R12, which its per-k-block FP32 scaling does not keep).
+// The decode kernel covers M <= 32 at g = 32 / 64 / 128, per-channel, and the group sizes in between whose
+// groups nest with its 16 warps' k ranges (one rounding per group, R12: their INT32 sums are combined before scaling).
 bool decode_supported(int M, int K, int g) {
   if (M > 32) return false;
-  return g == 32 || g == 64 || g == kBlockK || (g == K && K > kBlockK);
+  if (g == K && K <= kBlockK) return g == kBlockK;
+  return gemv_group_mode(K, g) >= 0;
 }
 
 int sm_count() {

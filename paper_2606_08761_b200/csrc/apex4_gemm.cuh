@@ -60,5 +60,6 @@ int gemm_max_pairs();
 // row blocks, upt = row blocks per shared-memory batch (<= gemv_max_batch(mt)), kbu = k-blocks per group.
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st);
 int gemv_max_batch(int mt);
+int gemv_group_mode(int K, int g);   // >= 0: the decode kernel covers this (K, g); -1: it does not
 
 }  // namespace apex4

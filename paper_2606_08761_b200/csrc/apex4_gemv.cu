@@ -87,16 +87,22 @@ struct GemvCfg {
   static_assert(kStageBytes % 16 == 0 && kSmemBytes <= 232448, "shared memory");
 };
 
-// CH: per-channel (one group = all of K).  The warps' k ranges are then parts of ONE group, so the
+// GM (group mode): 0 = a group is a k-block or a part of one (g <= 128): every k-block is scaled on its own;
+// 1 = a group is several k-blocks and a warp's k range is a whole number of groups (g = 256 .. with K / 16 a
+//     multiple of g): the INT32 sums of a group stay in registers across its k-blocks and are scaled once;
+// 2 = a warp's k range lies inside ONE group (per-channel g = K, or g a multiple of K / 16): see below.
+// GM = 2, e.g. per-channel (one group = all of K).  The warps' k ranges are then parts of ONE group, so the
 // partial sums stay INT32 through the k loop and through the cross-warp reduction (exact), and the two
 // scales are applied once at the end -- one rounding per group as R12 wants, which the per-k-block FP32
 // scaling of the g = 128 path cannot give for larger groups.  |256 P| <= 2^8 * 64 * 32768 = 2^29: no overflow.
 // GS > 1 (g = 64 / 32): lane (q, t) takes word t of each of the row's four 16-byte chunks instead of chunk t,
 // so that MMA c covers exactly k = 32 c .. 32 c + 31 of the k-block, i.e. one g = 32 group (half a g = 64
 // group), and every group gets its own scales.
-template <int MT, bool DUMP, bool CH, int GS>
+template <int MT, bool DUMP, int GM, int GS>
 __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams p) {
-  static_assert(!(CH && GS > 1), "per-channel has one group");
+  static_assert(GM == 0 || GS == 1, "groups of several k-blocks have no sub-k-block groups");
+  constexpr bool CH = GM == 2;          // INT32 partial sums meet across warps
+  const int kbpg = p.kbu;               // k-blocks per group (GM = 1, 2)
   using Cfg = GemvCfg<MT, GS>;
   constexpr int RBB = Cfg::RBB;
   extern __shared__ uint8_t smem_raw[];
@@ -135,7 +141,7 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
   // Source pointers advance by a blob (k-block) per stage and are set up once per batch: recomputing them
   // per stage cost ~120 (uniform-datapath) instructions per k-block.  One group per k-block (g = 128, the
   // only granularity the dispatcher sends here): group index = k-block index.
-  int ib0 = rb0, ij = 0, islot = 0;
+  int ib0 = rb0, ij = 0, islot = 0, ikin = 0;            // ikin: k-block inside its group (GM = 1)
   const uint8_t *w1 = nullptr, *w2 = nullptr, *aq = nullptr;
   const __half *s1 = nullptr, *s2 = nullptr, *sq = nullptr;
   uint32_t n1b = 0, n2b = 0, tx = 0;                    // rows x 64 bytes of the two pieces, bytes per stage
@@ -148,10 +154,12 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
     w1 = p.qW + tile_a * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes + (row_a & 127) * kRowBytes;
     w2 = p.qW + (tile_a + 1) * row_pitch + static_cast<size_t>(kbw0) * kBlobBytes;
     if constexpr (!CH && !DUMP) {   // the dump of the integer sums takes no scales (null pointers)
-      s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + GS * kbw0) * kTileRows + (row_a & 127);
-      s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + GS * kbw0) * kTileRows;
-      sq = p.sA + static_cast<size_t>(GS * kbw0) * kTileRows;
+      const int g0 = GM == 1 ? kbw0 / kbpg : GS * kbw0;               // first group of this warp's k range
+      s1 = p.sW + (static_cast<size_t>(tile_a) * p.G + g0) * kTileRows + (row_a & 127);
+      s2 = p.sW + (static_cast<size_t>(tile_a + 1) * p.G + g0) * kTileRows;
+      sq = p.sA + static_cast<size_t>(g0) * kTileRows;
     }
+    ikin = 0;
     aq = p.qA + static_cast<size_t>(kbw0) * kBlobBytes;
     n1b = n1 * kRowBytes;
     n2b = n2 * kRowBytes;
@@ -199,7 +207,10 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
       ++n_pre;
     }
     w1 += kBlobBytes; w2 += kBlobBytes; aq += kBlobBytes;
-    if constexpr (!CH && !DUMP) { s1 += GS * kTileRows; s2 += GS * kTileRows; sq += GS * kTileRows; }
+    if constexpr (!CH && !DUMP) {
+      // every k-block stage carries the scales of ITS group: the pointers move on at a group boundary
+      if (GM == 0 || ++ikin == kbpg) { s1 += GS * kTileRows; s2 += GS * kTileRows; sq += GS * kTileRows; ikin = 0; }
+    }
     islot = islot + 1 == kStages ? 0 : islot + 1;
     if (++ij == nkw) {
       ij = 0;
@@ -269,13 +280,14 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
           af[mi][i][0] = swap ? h0 : l0; af[mi][i][2] = swap ? l0 : h0;   // token q: k lo / hi half
           af[mi][i][1] = swap ? h1 : l1; af[mi][i][3] = swap ? l1 : h1;   // token q + 8
         }
-        if constexpr (!CH && GS == 1) {
+        if constexpr (GM != 2 && GS == 1) {
           const __half* sah = reinterpret_cast<const __half*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + Cfg::kSWBytes);
           sa[mi][0] = __half2float(sah[16 * mi + q]);
           sa[mi][1] = __half2float(sah[16 * mi + q + 8]);
         }
       }
       const int gm = DUMP ? (kbw0 + j) / p.kbu : 0;
+      const bool group_ends = GM == 1 && ((kbw0 + j + 1) % kbpg) == 0;   // warp ranges start on group boundaries
 #pragma unroll
       for (int i = 0; i < RBB; ++i) {
         if (i < nb) {
@@ -322,12 +334,35 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
             continue;
           }
           lds128(st + i * 512 + lane_off, x[0], x[1], x[2], x[3]);
-          if constexpr (CH) {
+          if constexpr (GM != 0) {
 #pragma unroll
             for (int k4 = 0; k4 < 4; ++k4) {
               const uint32_t b0w = rotl4(x[k4]) & kMask, b1w = x[k4] & kMask;
 #pragma unroll
               for (int mi = 0; mi < MT; ++mi) mma_s8(ia[i][mi], af[mi][k4], b0w, b1w);
+            }
+            if constexpr (GM == 1) {
+              if (group_ends) {     // the group's exact sum: INT32 -> FP32, x sW / 256, x sA, once (a5, R12)
+                const __half2 sw2 = *reinterpret_cast<const __half2*>(smem_gen + (st - smem_base) + Cfg::kWBytes + Cfg::kABytes + i * 16 + 4 * t);
+                const float sw0 = __low2float(sw2) * 0.00390625f, sw1 = __high2float(sw2) * 0.00390625f;
+#pragma unroll
+                for (int mi = 0; mi < MT; ++mi) {
+                  yf[i][mi][0] = fmaf(__int2float_rn(ia[i][mi][0]) * sw0, sa[mi][0], yf[i][mi][0]);
+                  yf[i][mi][1] = fmaf(__int2float_rn(ia[i][mi][1]) * sw1, sa[mi][0], yf[i][mi][1]);
+                  yf[i][mi][2] = fmaf(__int2float_rn(ia[i][mi][2]) * sw0, sa[mi][1], yf[i][mi][2]);
+                  yf[i][mi][3] = fmaf(__int2float_rn(ia[i][mi][3]) * sw1, sa[mi][1], yf[i][mi][3]);
+                  if constexpr (DUMP) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                      const int m = 16 * mi + q + 8 * (e >> 1), n = (b0 + i) * 8 + 2 * t + (e & 1);
+                      if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1)
+                        p.P_out[(static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gm] = ia[i][mi][e] >> 8;
+                    }
+                  }
+#pragma unroll
+                  for (int e = 0; e < 4; ++e) ia[i][mi][e] = 0;
+                }
+              }
             }
             continue;
           }
@@ -386,30 +421,35 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
           const int n = (b0 + i) * 8 + 2 * t;
           const int m = 16 * mi + q;
           if constexpr (CH) {
-            int s0 = 0, s1i = 0, s2i = 0, s3 = 0;         // exact: INT32 all the way
+            // the warps [gamma wpg, (gamma + 1) wpg) hold the parts of group gamma (all 16 for per-channel)
+            const int wpg = kWarps / p.G;
+            for (int gamma = 0; gamma < p.G; ++gamma) {
+              int s0 = 0, s1i = 0, s2i = 0, s3 = 0;         // exact: INT32 all the way
+              for (int ww = gamma * wpg; ww < (gamma + 1) * wpg; ++ww) {
+                const float4 xx = part[((i * kWarps + ww) * MT + mi) * 32 + lane];
+                s0 += __float_as_int(xx.x); s1i += __float_as_int(xx.y); s2i += __float_as_int(xx.z); s3 += __float_as_int(xx.w);
+              }
+              s0 >>= 8; s1i >>= 8; s2i >>= 8; s3 >>= 8;       // operands were 16 q each
+              if constexpr (DUMP) {
+                const int sums[4] = {s0, s1i, s2i, s3};
 #pragma unroll
-            for (int ww = 0; ww < kWarps; ++ww) {
-              const float4 xx = part[((i * kWarps + ww) * MT + mi) * 32 + lane];
-              s0 += __float_as_int(xx.x); s1i += __float_as_int(xx.y); s2i += __float_as_int(xx.z); s3 += __float_as_int(xx.w);
-            }
-            s0 >>= 8; s1i >>= 8; s2i >>= 8; s3 >>= 8;       // operands were 16 q each
-            if constexpr (DUMP) {
-              const int sums[4] = {s0, s1i, s2i, s3};
-#pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                const int mm = m + 8 * (e >> 1), nn = n + (e & 1);
-                if (mm >= p.pm0 && mm < p.pm1 && nn >= p.pn0 && nn < p.pn1)
-                  p.P_out[(static_cast<size_t>(mm - p.pm0) * (p.pn1 - p.pn0) + (nn - p.pn0)) * p.G] = sums[e];
+                for (int e = 0; e < 4; ++e) {
+                  const int mm = m + 8 * (e >> 1), nn = n + (e & 1);
+                  if (mm >= p.pm0 && mm < p.pm1 && nn >= p.pn0 && nn < p.pn1)
+                    p.P_out[(static_cast<size_t>(mm - p.pm0) * (p.pn1 - p.pn0) + (nn - p.pn0)) * p.G + gamma] = sums[e];
+                }
+              }
+              if constexpr (!DUMP) {   // the dump takes no scales (null pointers; the loads below may be hoisted)
+                if (p.Y != nullptr && n < p.N) {
+                  // Y += float(P) sW sA (a5), P exact in FP32 (|P| <= 64 K < 2^24): one rounding chain per group (R12)
+                  const float sw0 = __half2float(__ldg(p.sW + st16_index(n, gamma, p.G))), sw1 = __half2float(__ldg(p.sW + st16_index(n + 1, gamma, p.G)));
+                  const float sa0 = __half2float(__ldg(p.sA + st16_index(m, gamma, p.G))), sa1 = __half2float(__ldg(p.sA + st16_index(m + 8, gamma, p.G)));
+                  v.x += __int2float_rn(s0) * sw0 * sa0; v.y += __int2float_rn(s1i) * sw1 * sa0;
+                  v.z += __int2float_rn(s2i) * sw0 * sa1; v.w += __int2float_rn(s3) * sw1 * sa1;
+                }
               }
             }
             if (p.Y == nullptr || n >= p.N) continue;
-            if constexpr (!DUMP) {   // the dump takes no scales (null pointers; the loads below may be hoisted)
-              // one group: Y = float(P) sW sA (a5), P exact in FP32 (|P| <= 64 K < 2^24)
-              const float sw0 = __half2float(__ldg(p.sW + st16_index(n, 0, 1))), sw1 = __half2float(__ldg(p.sW + st16_index(n + 1, 0, 1)));
-              const float sa0 = __half2float(__ldg(p.sA + st16_index(m, 0, 1))), sa1 = __half2float(__ldg(p.sA + st16_index(m + 8, 0, 1)));
-              v.x = __int2float_rn(s0) * sw0 * sa0; v.y = __int2float_rn(s1i) * sw1 * sa0;
-              v.z = __int2float_rn(s2i) * sw0 * sa1; v.w = __int2float_rn(s3) * sw1 * sa1;
-            }
           } else {
 #pragma unroll
           for (int ww = 0; ww < kWarps; ++ww) {
@@ -436,39 +476,51 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <int MT, bool CH, int GS>
+template <int MT, int GM, int GS>
 static cudaError_t launch_gemv_m(const GemmParams& p, bool dump, int grid, cudaStream_t st) {
   constexpr int smem = GemvCfg<MT, GS>::kSmemBytes;
   cudaError_t e;
   if (dump) {
-    auto kern = w4a4_gemv_kernel<MT, true, CH, GS>;
+    auto kern = w4a4_gemv_kernel<MT, true, GM, GS>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     if ((e = launch_pdl(kern, dim3(grid), dim3(kThreads), smem, st, p)) != cudaSuccess) return e;
   } else {
-    auto kern = w4a4_gemv_kernel<MT, false, CH, GS>;
+    auto kern = w4a4_gemv_kernel<MT, false, GM, GS>;
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     if ((e = launch_pdl(kern, dim3(grid), dim3(kThreads), smem, st, p)) != cudaSuccess) return e;
   }
   return cudaGetLastError();
 }
 template <int MT>
-static cudaError_t launch_gemv_g(const GemmParams& p, bool ch, int gs, bool dump, int grid, cudaStream_t st) {
-  if (ch) return launch_gemv_m<MT, true, 1>(p, dump, grid, st);
-  if (gs == 4) return launch_gemv_m<MT, false, 4>(p, dump, grid, st);
-  if (gs == 2) return launch_gemv_m<MT, false, 2>(p, dump, grid, st);
-  return launch_gemv_m<MT, false, 1>(p, dump, grid, st);
+static cudaError_t launch_gemv_g(const GemmParams& p, int gm, int gs, bool dump, int grid, cudaStream_t st) {
+  if (gm == 2) return launch_gemv_m<MT, 2, 1>(p, dump, grid, st);
+  if (gm == 1) return launch_gemv_m<MT, 1, 1>(p, dump, grid, st);
+  if (gs == 4) return launch_gemv_m<MT, 0, 4>(p, dump, grid, st);
+  if (gs == 2) return launch_gemv_m<MT, 0, 2>(p, dump, grid, st);
+  return launch_gemv_m<MT, 0, 1>(p, dump, grid, st);
+}
+
+// Group mode of the decode kernel for (K, g), or -1 if it does not cover them (see the kernel's GM comment):
+// 16 warps split the K / 128 k-blocks evenly; groups of several k-blocks must nest with those ranges.
+int gemv_group_mode(int K, int g) {
+  const int KB = K / kBlockK;
+  if (g <= kBlockK) return (g == 32 || g == 64 || g == kBlockK) ? 0 : -1;
+  if (g == K) return 2;                                   // per-channel: every warp inside the one group, any KB
+  if (g % kBlockK != 0 || KB % gemv::kWarps != 0) return -1;
+  const int q = KB / gemv::kWarps, kbpg = g / kBlockK;
+  if (q % kbpg == 0) return 1;
+  if (kbpg % q == 0 && gemv::kWarps % (K / g) == 0) return 2;
+  return -1;
 }
 
 // mt: m16 token tiles (1 or 2)
 cudaError_t launch_gemv(const GemmParams& p, int mt, bool dump, int grid, cudaStream_t st) {
-  // one group per k-block (g = 128), or one group for all of K (per-channel, exact INT32 reduction)
-  const bool ch = p.G == 1 && p.K > kBlockK;
-  if (!ch && p.kbu != 1) return cudaErrorInvalidValue;
+  const int gm = gemv_group_mode(p.K, p.g);
+  if (gm < 0) return cudaErrorInvalidValue;
   const int gs = p.g < kBlockK ? kBlockK / p.g : 1;     // groups per k-block (g = 64: 2, g = 32: 4)
-  if (gs != 1 && gs != 2 && gs != 4) return cudaErrorInvalidValue;
   switch (mt) {
-    case 1: return launch_gemv_g<1>(p, ch, gs, dump, grid, st);
-    case 2: return launch_gemv_g<2>(p, ch, gs, dump, grid, st);
+    case 1: return launch_gemv_g<1>(p, gm, gs, dump, grid, st);
+    case 2: return launch_gemv_g<2>(p, gm, gs, dump, grid, st);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -103,9 +103,14 @@ def test_dispatch_table(L):
     # per-channel decode: the streaming kernel with an exact INT32 cross-warp reduction, no workspace
     assert apex4.debug_get_dispatch(16, 8192, 8192, 0, apex4.GRAN_CHANNEL)[:3] == (DEC, 16, 0)
     assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0
-    # groups between 128 and K at small M: CTA pairs on 256 x 64 tiles; a group is the indivisible k unit
-    kern, width, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 8192, 1024)
-    assert (kern, width, upt) == (PAIR, 64, 8)
+    # groups between 128 and K at small M: the decode kernel where the groups nest with its 16 warps' k ranges
+    # (K / 16 a multiple of g, or g a multiple of K / 16 with K / g dividing 16), CTA pairs on 256 x 64 tiles otherwise
+    for g in (256, 512, 1024, 2048, 4096):
+        assert apex4.debug_get_dispatch(16, 8192, 8192, g)[0] == DEC
+    assert apex4.debug_get_dispatch(16, 8192, 28672, 256)[0] == DEC
+    kern, width, split, grid, upt = apex4.debug_get_dispatch(16, 8192, 28672, 1024)      # 224 k-blocks: 14 per warp, 8 per group
+    assert (kern, width, upt) == (PAIR, 64, 28)
+    assert apex4.debug_get_dispatch(16, 4096, 11008, 256)[0] == PAIR                      # 86 k-blocks do not split over 16 warps
     # per-call options: forcing the pair kernel / a tile width / stream-K changes this call only
     o = apex4.debug_opts(kernel=PAIR, pair_tokens=128, split=1, grid=5)
     assert apex4.debug_get_dispatch(16, 256, 512, 128, opts=o)[:4] == (PAIR, 128, 1, 4)   # 4 units: grid capped
@@ -113,5 +118,5 @@ def test_dispatch_table(L):
     assert apex4.debug_get_dispatch(16, 256, 512, 128)[0] == DEC                           # ... not the next one
     with pytest.raises(apex4.Apex4Error):            # the decode kernel does not cover M > 32
         apex4.debug_get_dispatch(64, 256, 512, 128, opts=apex4.debug_opts(kernel=DEC))
-    with pytest.raises(apex4.Apex4Error):            # ... nor groups between 128 and K
+    with pytest.raises(apex4.Apex4Error):            # ... nor groups that do not nest with its warps' k ranges
         apex4.debug_get_dispatch(16, 256, 1024, 256, opts=apex4.debug_opts(kernel=DEC))

@@ -230,6 +230,20 @@ def test_gemm_pair_tile_widths(A, M, N, K, g, opts):
     run_gemm_case(A, M, N, K, g, seed=500 + M, opts=opts, out_f32=True, sums=None)
 
 
+@pytest.mark.parametrize("M,N,K,g", [(16, 264, 8192, 256), (16, 264, 8192, 512), (9, 136, 8192, 1024), (32, 264, 8192, 2048),
+                                     (20, 136, 4096, 256), (17, 136, 4096, 512), (5, 72, 4096, 1024), (3, 64, 28672, 256),
+                                     (16, 264, 2048, 256), (31, 264, 2048, 1024)])
+@pytest.mark.parametrize("grid", [0, 3])
+def test_gemm_decode_groups_between_128_and_K(A, M, N, K, g, grid):
+    """Decode (M <= 32) at 128 < g < K (the paper's granularities 256 / 512 / 1024): a group's INT32 sum
+    is completed before it is scaled -- inside a warp when its k range holds whole groups, across warps through
+    shared memory when several warps share a group -- so every group is rounded once (R12)."""
+    assert A.debug_get_dispatch(M, N, K, g)[0] == DECODE
+    run_gemm_case(A, M, N, K, g, seed=850 + M, opts=dict(kernel=DECODE, grid=grid))
+    run_gemm_case(A, M, N, K, g, seed=850 + M, opts=dict(kernel=DECODE, grid=grid), out_f32=True, sums=None)
+    run_gemm_case(A, M, N, K, g, seed=850 + M, opts=dict(kernel=PAIR), sums=None)       # the pair kernel agrees
+
+
 def test_gemm_decode_f32_and_large_group_routing(A):
     run_gemm_case(A, 16, 256, 1024, 128, seed=7, out_f32=True, opts=dict(kernel=DECODE))
     # groups larger than a k-block keep one rounding per group: the pair kernel handles them
