@@ -203,6 +203,14 @@ int apex4_debug_get_dispatch(int M, int N, int K, int group_size, int gran, int 
  * does). */
 int apex4_measure_rho(double* out_host, void* stream);
 
+/* The Blackwell form of the paper's Tensor-Core / CUDA-Core tension inside the epilogue (a5): how much the TMEM
+ * <-> register traffic of the dequant step (tcgen05.ld of the accumulators, tcgen05.st of the magic bias) and its
+ * FP32 FMAs slow each other down on one SM.  out_host (HOST, >= 16 doubles): for mode m = 1..7 (bit 0 loads, bit 1
+ * stores, bit 2 FFMA2) out[2m] = clocks a TMEM warp needs per 16 accumulator columns, out[2m+1] = clocks an FFMA2
+ * warp needs per 32 FFMA2 (the FMAs of 16 columns), two warps of each kind per SM sub-partition.  Synchronises the
+ * stream; allocates and frees ~2 KB of device scratch. */
+int apex4_measure_epilogue_pipes(double* out_host, void* stream);
+
 /* ---- experiment: is an FP8 tensor-core path exact on INT4 codes? ------------------------------- */
 /* Runs one 128 x 256 tile over K (multiple of 128, <= 32768) through tcgen05.mma kind::i8 and through
  * kind::f8f6f4 with the same codes as E4M3 operands and compares the two TMEM accumulators element by element.

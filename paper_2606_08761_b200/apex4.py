@@ -30,7 +30,8 @@ EXPORTS = (
     "apex4_rmsnorm_quantize", "apex4_silu_mul_quantize",
     "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
     "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes",
-    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_e4m3_exactness",
+    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_measure_epilogue_pipes",
+    "apex4_e4m3_exactness",
 )
 
 
@@ -108,6 +109,8 @@ def lib() -> ctypes.CDLL:
     L.apex4_debug_group_sums.argtypes = [c_void_p, c_void_p] + [c_int] * 10 + [c_void_p, c_void_p,
                                                                               ctypes.POINTER(DebugOpts)]
     L.apex4_measure_rho.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
+    L.apex4_measure_epilogue_pipes.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
+    L.apex4_measure_epilogue_pipes.restype = c_int
     L.apex4_e4m3_exactness.argtypes = [c_int, c_int, c_int, ctypes.c_uint, ctypes.POINTER(ctypes.c_double), c_void_p]
     L.apex4_e4m3_exactness.restype = c_int
     L.apex4_debug_get_dispatch.argtypes = [c_int] * 6 + [ctypes.POINTER(DebugOpts), ctypes.POINTER(c_int)]
@@ -324,6 +327,15 @@ def measure_rho() -> dict:
     keys = ("int8_tops", "fp32_tflops", "i2f_gops", "rho", "tmem_ld_gbs", "sm_clock_mhz",
             "int8_mac_per_clk_sm", "tmem_ld_bytes_per_clk_sm")
     return dict(zip(keys, [float(v) for v in out]))
+
+
+def measure_epilogue_pipes() -> dict:
+    """apex4_measure_epilogue_pipes: clocks per 16 accumulator columns (TMEM warp) / per 32 FFMA2 (FFMA2 warp) with
+    tcgen05.ld, tcgen05.st and FFMA2 streams alone and together."""
+    out = (ctypes.c_double * 16)()
+    _check(lib().apex4_measure_epilogue_pipes(out, _stream()), "apex4_measure_epilogue_pipes")
+    names = {1: "ld", 2: "st", 3: "ld+st", 4: "ffma2", 5: "ld|ffma2", 6: "st|ffma2", 7: "ld+st|ffma2"}
+    return {names[m]: {"tmem_clk_per_16_columns": float(out[2 * m]), "ffma2_clk_per_32": float(out[2 * m + 1])} for m in range(1, 8)}
 
 
 def e4m3_exactness(K: int, pattern: int, encoding: int, seed: int = 0) -> dict:

@@ -27,23 +27,42 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found (needed to build libapex4.so for sm_100a)")
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def _source_hash(extra=()) -> str:
+    """SHA-256 over every file under csrc/, include/apex4.h, the nvcc version and the flags: a library built from other
+    sources (a stale prebuilt .so that travelled with a snapshot) is rebuilt, whatever the file times say."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(CSRC)):
+        h.update(f.encode())
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    h.update(open(os.path.join(os.path.dirname(PKG), "include", "apex4.h"), "rb").read())
+    try:
+        h.update(subprocess.run([_nvcc(), "--version"], capture_output=True, text=True).stdout.encode())
+    except OSError:
+        pass
+    h.update(" ".join(NVCC_FLAGS + list(extra)).encode())
+    return h.hexdigest()
+
+
+def needs_build(lib: str = LIB, extra=()) -> bool:
+    stamp = lib + ".sha256"
+    if not os.path.exists(lib) or not os.path.exists(stamp):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps.append(os.path.join(os.path.dirname(PKG), "include", "apex4.h"))
-    return any(os.path.getmtime(d) > t for d in deps)
+    return open(stamp).read().strip() != _source_hash(extra)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compiles every source to an object file (in parallel) and links libapex4.so."""
-    if not force and not needs_build():
-        return LIB
+def build(force: bool = False, verbose: bool = False, out: str = LIB, defines=()) -> str:
+    """Compiles every source to an object file (in parallel) and links the library.  `defines` (e.g.
+    ["-DAPEX4_TIMELINE"], the tuning switches named in profiles/) and `out` build a variant next to the product
+    library (load it with APEX4_LIB=<out>); the default builds paper_2606_08761_b200/libapex4.so."""
+    defines = list(defines)
+    if not force and not needs_build(out, defines):
+        return out
     from concurrent.futures import ThreadPoolExecutor
-    objdir = os.path.join(PKG, "_obj")
+    tag = "" if out == LIB else "_" + os.path.splitext(os.path.basename(out))[0]
+    objdir = os.path.join(PKG, "_obj" + tag)
     os.makedirs(objdir, exist_ok=True)
-    base = [_nvcc()] + [f for f in NVCC_FLAGS if f != "--shared"] + (["-Xptxas", "-v"] if verbose else [])
+    base = [_nvcc()] + [f for f in NVCC_FLAGS if f != "--shared"] + defines + (["-Xptxas", "-v"] if verbose else [])
 
     def compile_one(src):
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
@@ -58,13 +77,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError(f"nvcc failed on {src}")
         if verbose:
             sys.stderr.write(res.stderr)
-    link = [_nvcc(), "--shared", "-gencode", "arch=compute_100a,code=sm_100a"] + [o for _, o, _ in results] + ["-o", LIB]
+    link = [_nvcc(), "--shared", "-gencode", "arch=compute_100a,code=sm_100a"] + [o for _, o, _ in results] + ["-o", out]
     res = subprocess.run(link, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("nvcc failed linking libapex4.so")
-    return LIB
+        raise RuntimeError("nvcc failed linking " + out)
+    with open(out + ".sha256", "w") as f:
+        f.write(_source_hash(defines) + "\n")
+    return out
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    # python -m paper_2606_08761_b200.build [--force] [-v] [--out PATH] [-DNAME[=VALUE] ...]
+    args = sys.argv[1:]
+    out = LIB
+    if "--out" in args:
+        out = os.path.abspath(args[args.index("--out") + 1])
+    print(build(force="--force" in args, verbose="-v" in args, out=out, defines=[a for a in args if a.startswith("-D")]))

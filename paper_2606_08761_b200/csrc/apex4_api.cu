@@ -23,6 +23,7 @@ cudaError_t launch_unpack_codes(const void* q, int R, int K, int8_t* codes, int 
 cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tiled, cudaStream_t st);
 cudaError_t launch_scales_to_natural(const void* tiled, int R, int G, void* nat, cudaStream_t st);
 int measure_rho(double* out, cudaStream_t st);
+int measure_epilogue_pipes(double* out, cudaStream_t st);
 int e4m3_exactness(int K, int pattern, int encoding, uint32_t seed, double* out, cudaStream_t st);
 }  // namespace apex4
 
@@ -453,6 +454,13 @@ int apex4_e4m3_exactness(int K, int pattern, int encoding, unsigned seed, double
   const int a = check_arch();
   if (a != APEX4_OK) return a;
   return e4m3_exactness(K, pattern, encoding, seed, out_host, static_cast<cudaStream_t>(stream));
+}
+
+int apex4_measure_epilogue_pipes(double* out_host, void* stream) {
+  if (!out_host) return APEX4_ERR_INVALID_ARG;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return measure_epilogue_pipes(out_host, static_cast<cudaStream_t>(stream));
 }
 
 int apex4_measure_rho(double* out_host, void* stream) {

@@ -607,7 +607,11 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           if (kVBufs == 2 && c < kChunks - 1) tmem_ld_32x16(tb + 16 * (c + 1), v[(c + 1) % kVBufs]);
 #endif
 #ifndef APEX4_X_NOSTTM
+#ifdef APEX4_X_HYBRID   // timing experiment (wrong results): warpgroup 1 on the I2F path, no re-bias
+          if (BIAS && h == 0) {
+#else
           if constexpr (BIAS) {
+#endif
             tmem_st_32x8(tb + 16 * c, mg);
             tmem_st_32x8(tb + 16 * c + 8, mg);
           }
@@ -642,7 +646,11 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
 #pragma unroll
           for (int jj = 0; jj < 8; ++jj) {
             uint64_t t0;
+#ifdef APEX4_X_HYBRID
+            if (h == 0) {
+#else
             if constexpr (BIAS) {
+#endif
 #ifdef APEX4_X_FMAINDEP
               t0 = fma2v(pack_u2(mg[jj & 7], mg[(jj + 1) & 7]), ab[0], ab[1]);
 #else

@@ -114,6 +114,84 @@ __global__ void __launch_bounds__(128, 1) mma_rate_kernel(int mma_iters, int ld_
   if (threadIdx.x < 32) { tc_fence_after(); tmem_dealloc<512>(tmem); }
 }
 
+// Epilogue-pipe interference probe (profiles/r2_gemm_pair_ncu.md): 16 warps on every SM; warps 0-7 stream the
+// TMEM traffic of the pair kernel's epilogue (tcgen05.ld 32x32b.x16 + wait and / or two tcgen05.st 32x32b.x8 per 16
+// columns), warps 8-15 a chain-free FFMA2 stream (32 per 16 columns, the two FMAs per element pair).  mode bit 0 =
+// loads, bit 1 = stores, bit 2 = FFMA2.  out[0] / out[1] = clocks of a TMEM warp / an FFMA2 warp.
+__global__ void __launch_bounds__(512, 1) epilogue_pipes_kernel(int mode, int iters, long long* out, float* sink) {
+  __shared__ uint32_t tptr;
+  const int warp = threadIdx.x >> 5;
+  if (warp == 0) tmem_alloc<512>(smem_u32(&tptr));
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tptr + (static_cast<uint32_t>((warp & 3) * 32) << 16);
+  const bool do_ld = mode & 1, do_st = mode & 2, do_fma = mode & 4;
+  const long long t0 = clock64();
+  if (warp < 8) {
+    uint32_t v[16], acc = 0, m[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) m[i] = 0x4B400000u + i;
+    for (int it = 0; it < iters; ++it) {
+      const uint32_t a = tb + (warp >> 2) * 96 + (it % 6) * 16;
+      if (do_ld) { tmem_ld_32x16(a, v); tmem_ld_wait16(v); acc ^= v[0] ^ v[7] ^ v[15]; }
+      if (do_st) { tmem_st_32x8(a, m); tmem_st_32x8(a + 8, m); }
+    }
+    if (do_st) tmem_st_wait();
+    sink[threadIdx.x] = __uint_as_float(acc);
+  } else if (do_fma) {
+    uint64_t a[8];
+    const uint64_t b2 = pack_f2(1.0001f, 0.9999f), c2 = pack_f2(0.5f, 0.25f);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = pack_f2(threadIdx.x * 0.001f + j, 1.f + j);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = fma2(a[j], b2, c2);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { float lo, hi; unpack_f2(a[j], lo, hi); s += lo + hi; }
+    sink[threadIdx.x] = s;
+  }
+  const long long t1 = clock64();
+  if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (warp == 0 || warp == 8)) out[warp >> 3] = t1 - t0;
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) { tc_fence_after(); tmem_dealloc<512>(tptr); }
+}
+
+int measure_epilogue_pipes(double* out, cudaStream_t st) {
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  long long* cyc = nullptr;
+  float* sink = nullptr;
+  if (cudaMalloc(&cyc, 2 * sizeof(long long)) != cudaSuccess) return APEX4_ERR_CUDA;
+  if (cudaMalloc(&sink, 512 * sizeof(float)) != cudaSuccess) { cudaFree(cyc); return APEX4_ERR_CUDA; }
+  const int iters = 3000;
+  int rc = APEX4_OK;
+  // out[2 m], out[2 m + 1], m = 1..7: clocks per 16 columns of a TMEM warp / per 32 FFMA2 of an FFMA2 warp in mode m
+  for (int i = 0; i < 16; ++i) out[i] = 0.0;
+  for (int mode = 1; mode < 8 && rc == APEX4_OK; ++mode) {
+    for (int rep = 0; rep < 2; ++rep) {
+      cudaMemsetAsync(cyc, 0, 2 * sizeof(long long), st);
+      epilogue_pipes_kernel<<<sms, 512, 0, st>>>(mode, iters, cyc, sink);
+    }
+    long long h[2];
+    if (cudaMemcpyAsync(h, cyc, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
+      rc = APEX4_ERR_CUDA;
+      break;
+    }
+    out[2 * mode] = (mode & 3) ? static_cast<double>(h[0]) / iters : 0.0;
+    out[2 * mode + 1] = (mode & 4) ? static_cast<double>(h[1]) / iters : 0.0;
+  }
+  cudaFree(cyc);
+  cudaFree(sink);
+  return cudaGetLastError() == cudaSuccess ? rc : APEX4_ERR_CUDA;
+}
+
 __global__ void clock_probe_kernel(long long* out) {
   unsigned long long g0, g1;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));

@@ -217,3 +217,69 @@ def run_sweeps(dev, peaks=None):
          "ratio": round(f11[(M, 128)]["us"] / f11[(M, 8192)]["us"], 3)}
         for M in sorted({k[0] for k in f11})]
     return res
+
+
+def render_markdown(d: dict, title: str) -> str:
+    """bench.py --sweep JSON line (dict) -> the markdown tables committed under profiles/."""
+    L = [f"# {title}", ""]
+    r = d["roofline"]
+    L.append(f"Headline (config 1, M=2048 Llama-2-7B linears, step = quantize + GEMM per layer): **{d['value']:.1f} TOPS**, "
+             f"{d['ms_per_step']:.3f} ms/step; GEMM launches alone {r['achieved']:.1f} TOP/s = {r['frac']:.3f} of {r['peak']:.0f} TOP/s "
+             f"({r['peak_source']}), {r['frac_of_spec_4500_tops']:.3f} of the 4.5 POPS datasheet figure; e2e {d['e2e']['value']:.1f} TOPS; "
+             f"clocks {d['clocks']['sm_mhz']} MHz of {d['clocks']['sm_max_mhz']}, reasons {d['clocks']['reasons']}; "
+             f"output check {d.get('check')}; cpu_baseline {d.get('cpu_baseline', {}).get('value', float('nan')):.4f} TOPS on "
+             f"{d.get('cpu_baseline', {}).get('cores')} cores.")
+    L.append("")
+    L.append("Per layer: " + "; ".join(f"{k}: GEMM {v['gemm_ms'] * 1e3:.0f} us = {v['gemm_tops']:.0f} TOPS, quantizer {v['quant_ms'] * 1e3:.1f} us = "
+                                       f"{v['quant_gbs']:.0f} GB/s" for k, v in r["per_layer"].items()))
+    L.append("")
+    if "targets" in r:
+        L.append("Target points of BASELINE.json (" + r.get("targets_protocol", "") + "):")
+        L.append("")
+        L.append("| M | N | K | g | kernel | GEMM us | quant+GEMM us | achieved | bound | frac of measured peak | frac of datasheet | cuBLAS FP16 us | speed-up (GEMM) | speed-up (quant+GEMM) |")
+        L.append("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+        for t in r["targets"]:
+            L.append(f"| {t['M']} | {t['N']} | {t['K']} | {t['g']} | {t['kernel']} | {t['us']} | {t['us_with_quant']} | {t['achieved']:.1f} {t['unit']} | {t['bound']} | "
+                     f"{t['frac']:.3f} | {t['frac_of_spec']:.3f} | {t['cublas_fp16_us']} | {t['speedup_vs_cublas_fp16']} | {t['speedup_vs_cublas_fp16_with_quant']} |")
+        L.append("")
+        if "rho" in r:
+            rh = r["rho"]
+            L.append(f"rho microbenchmark in the same run: INT8 {rh['int8_tops']:.0f} TOPS ({rh['int8_mac_per_clk_sm']:.0f} MAC/clk/SM), FP32 {rh['fp32_tflops']:.1f} TFLOP/s, "
+                     f"rho = {rh['rho']:.1f}, TMEM read {rh['tmem_ld_bytes_per_clk_sm']:.0f} B/clk/SM, SM clock {rh['sm_clock_mhz']:.0f} MHz.")
+            L.append("")
+    sw = d.get("sweep")
+    if sw:
+        L.append("Sweeps: " + sw["protocol"])
+        L.append("")
+        L.append("| config | M | N | K | g | kernel | us | eff. TOPS | GB/s (algorithmic) | bound | frac of peak | cuBLAS FP16 us | speed-up |")
+        L.append("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+        for tag, key in (("2", "config2_square_sweep"), ("3", "config3_granularity"), ("4", "config4_llama70b")):
+            for x in sw[key]:
+                fr = x.get("frac_of_int8_peak", x.get("frac_of_hbm_peak", ""))
+                L.append(f"| {tag} | {x['M']} | {x['N']} | {x['K']} | {x['g']} | {x['kernel']} | {x['us']} | {x['tops']} | {x['gbs']} | {x.get('bound', '')} | {fr} | "
+                         f"{x.get('cublas_fp16_us', '')} | {x.get('speedup_vs_cublas_fp16', '')} |")
+        L.append("")
+        m = sw["config3_mixed"]
+        L.append(f"Config 3 mixed granularity (R11, two fine + five per-channel linears per block mapped onto the 4096 x 8192 x 8192 shape): paper mix (fine = 32) "
+                 f"{m['paper_mix_fine32_us']} us, BASELINE wording (fine = 128) {m['baseline_mix_fine128_us']} us, uniform g128 {m['uniform_g128_us']} us.")
+        L.append("")
+        L.append("Fig. 11 (PAPER.md:361-363), N = K = 8192, time of g = 128 over per-channel: " +
+                 "; ".join(f"M={x['M']}: {x['g128_us']} / {x['channel_us']} us = {x['ratio']}" for x in sw["fig11_g128_over_channel"]) + ".")
+        L.append("")
+        L.append("Whole transformer block (every quantizer call + GEMM; G_a = G_w so the paper's mix quantizes the block input twice and splits V off QKV):")
+        L.append("")
+        L.append("| model | M | policy | block us | eff. TOPS | ops (us) |")
+        L.append("|---|---|---|---|---|---|")
+        for b in sw["block_policies"]:
+            ops = ", ".join(f"{o['op']}@g{o['g']} {o['us']}" for o in b["ops"])
+            L.append(f"| {b['model']} | {b['M']} | {b['policy']} | {b['block_us']} | {b['tops']} | {ops} |")
+        L.append("")
+    return "\n".join(L) + "\n"
+
+
+if __name__ == "__main__":
+    # python -m paper_2606_08761_b200.sweep <bench.json> "<title>"  ->  markdown on stdout
+    import json
+    import sys
+    line = [l for l in open(sys.argv[1]) if l.startswith("{")][-1]
+    sys.stdout.write(render_markdown(json.loads(line), sys.argv[2] if len(sys.argv) > 2 else "bench.py --sweep"))
