@@ -57,6 +57,14 @@ constexpr uint32_t kMagicBits = 0x4B400000u;   // float 12582912 = 1.5 * 2^23
 #define APEX4_EPI_WGS_192 2          // epilogue warpgroups of the 192-token tile (tuning builds: 3)
 #endif
 constexpr int kAccBufs = 2;
+#ifndef APEX4_X_HALVES
+#define APEX4_X_HALVES 1
+#endif
+// Tuning option (2): each accumulator buffer is produced as two independent column halves -- one MMA of N = NT / 2
+// and one full / empty barrier pair per half -- so that the two epilogue warpgroups hand their halves back and
+// get them refilled independently.  Measured slower than one MMA per buffer (profiles/r2_gemm_pair_ncu.md): the
+// epilogue is bound by its own instruction stream, not by the hand-off.
+constexpr int kHalves = APEX4_X_HALVES;
 constexpr int kOpStages = 4;        // widened operand stages (TMEM A + smem B)
 constexpr int kPkStages = 6;        // packed (bulk copy) stages
 constexpr int kScfSlots = 8;
@@ -64,7 +72,7 @@ constexpr int kTmemA0 = 384;        // first TMEM column of the A-operand stages
 constexpr int kPkWBytes = kBlobBytes;             // 128 weight rows of a k-block
 constexpr int kPkSWBytes = 4 * 256;               // up to 4 groups per k-block, 128 FP16 each
 constexpr int kPkSABytes = 2 * 4 * 256;           // the (up to) two 128-token blobs the tile touches
-constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs;
+constexpr int kNumBars = 2 * kPkStages + 2 * kOpStages + 2 * kScfSlots + 2 * kAccBufs * kHalves;
 static_assert((kScfSlots & (kScfSlots - 1)) == 0, "power-of-two wraps");
 static_assert((kOpStages & (kOpStages - 1)) == 0, "stage index wraps with a mask");
 
@@ -120,6 +128,10 @@ struct Tile {
   static_assert(kSmemBytes <= 232448, "shared memory");
   static_assert(NT % (16 * kEpiWGs) == 0, "epilogue warpgroups own whole 16-column chunks");
   static_assert(kChunks % 2 == 0, "the cross-group prefetch lands in v[0] while the last (odd) chunk is in v[1]");
+  static constexpr int kPieceRows = kHalf / kHalves;    // token rows per CTA and accumulator half
+  static constexpr int kMmaN = NT / kHalves;
+  static_assert(kHalves == 1 || kEpiWGs == kHalves, "one epilogue warpgroup per accumulator half");
+  static_assert(kPieceRows % 8 == 0 && kMmaN % 16 == 0, "swizzle atoms / MMA N of a half");
 };
 
 // Warp layout for WWG widener warpgroups.  With one, the wideners of a CTA run one k-block at a time:
@@ -136,11 +148,20 @@ struct Warps {
   static constexpr int kCtlWarp0 = kEpiWarp0 + kEpiWarps;   // producer warp; the MMA warp follows
   static constexpr int kThreads = 32 * (kCtlWarp0 + 4);     // warps are allocated in fours: two control warps idle
   static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8;
-  static constexpr int kRegsCtl = 32, kRegsWiden = WWG == 1 ? 64 : 56;
+  // control 24 (the minimum; the producer spills two work-iterator words, off the critical path), wideners 56:
+  // with one widener warpgroup that leaves 216 for the epilogue, whose group loop (96 FP32 accumulators, two 16-column
+  // TMEM chunks, 16 token scales, the magic bias) spills at 208 -- 414 us against 368 us at M = 4096, N = K = 8192
+  // (with two widener warpgroups the epilogue gets 168 either way, and the control warps keep 32)
+  static constexpr int kRegsCtl = WWG == 1 ? 24 : 32, kRegsWiden = 56;
   static constexpr int kRegsEpi = ((kThreads * kLaunchRegs - 128 * kRegsCtl - 128 * WWG * kRegsWiden) / (128 * kEpiWGs)) / 8 * 8;
   static_assert((WWG & (WWG - 1)) == 0, "k-blocks are dealt with a mask");
   static_assert(128 * kRegsCtl + 128 * WWG * kRegsWiden + 128 * kEpiWGs * kRegsEpi <= kThreads * kLaunchRegs, "registers");
   static_assert(kRegsEpi <= 232 && kThreads <= 1024, "register / thread limits");
+};
+
+// "a group follows" as a compile-time fact of one copy of the epilogue's group body
+struct Always {
+  __device__ constexpr operator bool() const { return true; }
 };
 
 struct Work {
@@ -198,6 +219,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
   constexpr bool kScfSync = GR::kScfSync;
   constexpr int kNT = T::kNT, kHalf = T::kHalf, kEpiCols = T::kEpiCols, kChunks = T::kChunks;
   constexpr int kEpiWarps = T::kEpiWarps;
+  constexpr int kPieceRows = T::kPieceRows;
   constexpr int kPkABytes = T::kPkABytes, kPkStageBytes = T::kPkStageBytes, kI8StageBytes = T::kI8StageBytes;
   constexpr int kScfSlotBytes = T::kScfSlotBytes, kStoreBytes = T::kStoreBytes, kTokIters = T::kTokIters;
   constexpr int kWidenWGs = L::kWidenWGs, kEpiWarp0 = L::kEpiWarp0, kCtlWarp0 = L::kCtlWarp0;
@@ -220,7 +242,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
   constexpr int bPkFull = 0, bPkEmpty = bPkFull + kPkStages, bOpFull = bPkEmpty + kPkStages,
                 bOpEmpty = bOpFull + kOpStages, bScfFull = bOpEmpty + kOpStages,
                 bScfEmpty = bScfFull + kScfSlots, bAccFull = bScfEmpty + kScfSlots,
-                bAccEmpty = bAccFull + kAccBufs;
+                bAccEmpty = bAccFull + kAccBufs * kHalves;   // index: buffer * kHalves + half
 
   // warp index through a shuffle from lane 0: tells the compiler it is warp-uniform, so addresses derived
   // from it (TMEM lane quarter, barrier and stage addresses) live in uniform registers (no R2UR per use)
@@ -238,7 +260,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
     for (int i = 0; i < kOpStages; ++i) { mbar_init(bar(bOpFull + i), 8); mbar_init(bar(bOpEmpty + i), 1); }
     for (int i = 0; i < kScfSlots; ++i) { mbar_init(bar(bScfFull + i), 128); mbar_init(bar(bScfEmpty + i), kEpiWarps); }
     // accumulator buffer empty: one elected arrive per epilogue warp of BOTH CTAs, on the leader's barrier
-    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 2 * kEpiWarps); }
+    for (int i = 0; i < kAccBufs * kHalves; ++i) { mbar_init(bar(bAccFull + i), 1); mbar_init(bar(bAccEmpty + i), 2 * kEpiWarps / kHalves); }
     fence_mbar_init();
   }
   if (threadIdx.x < 8) reinterpret_cast<volatile uint32_t*>(smem_gen + offMagic)[threadIdx.x] = kMagicBits;
@@ -276,20 +298,29 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
       while (work_next(p, wit, w, cp, npairs)) {
         const int wblob = 2 * w.nt + static_cast<int>(rank);
         const bool has_w = wblob < n_blobs;
-        // this CTA's token rows: up to two pieces of consecutive blobs
-        const int t0 = w.mt * kNT + static_cast<int>(rank) * kHalf;
-        const int ab0 = t0 >> 7, ar0 = t0 & 127;
-        const int n1 = ab0 < m_blobs ? min(kHalf, kTileRows - ar0) : 0;
-        const int n2 = (ab0 + 1 < m_blobs) ? kHalf - min(kHalf, kTileRows - ar0) : 0;
+        // this CTA's token rows: accumulator half hh covers tile tokens [hh * kMmaN, (hh + 1) * kMmaN), of which
+        // this CTA supplies kPieceRows (the MMA takes N / 2 rows of B from each CTA); a piece may straddle two blobs
+        int ar0[kHalves], n1[kHalves], n2[kHalves];
+        const uint8_t* asrc[kHalves];
+        uint32_t arows = 0;
+#pragma unroll
+        for (int hh = 0; hh < kHalves; ++hh) {
+          const int t0 = w.mt * kNT + hh * T::kMmaN + static_cast<int>(rank) * kPieceRows;
+          const int ab0 = t0 >> 7;
+          ar0[hh] = t0 & 127;
+          n1[hh] = ab0 < m_blobs ? min(kPieceRows, kTileRows - ar0[hh]) : 0;
+          n2[hh] = (ab0 + 1 < m_blobs) ? kPieceRows - min(kPieceRows, kTileRows - ar0[hh]) : 0;
+          asrc[hh] = p.qA + ab0 * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes + ar0[hh] * kRowBytes;
+          arows += n1[hh] + n2[hh];
+        }
         // token scales: the two blobs the tile touches
         const int sb0 = (w.mt * kNT) >> 7;
         const int s_blobs = min((((w.mt * kNT) & 127) + kNT > kTileRows) ? 2 : 1, m_blobs - sb0);
         const int gfirst0 = GR::kMultiKb ? w.kb0 / kbpg : w.kb0 * GPK;
         const uint8_t* wsrc = p.qW + wblob * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes;
-        const uint8_t* asrc = p.qA + ab0 * row_pitch + static_cast<size_t>(w.kb0) * kBlobBytes + ar0 * kRowBytes;
         const __half* swsrc = p.sW + wblob * srow_pitch + static_cast<size_t>(gfirst0) * kTileRows;
         const __half* sasrc = p.sA + sb0 * srow_pitch + static_cast<size_t>(gfirst0) * kTileRows;
-        const uint32_t bytes_data = (has_w ? kBlobBytes : 0) + (n1 + n2) * kRowBytes;
+        const uint32_t bytes_data = (has_w ? kBlobBytes : 0) + arows * kRowBytes;
         const uint32_t bytes_scales = sc_bytes * ((has_w ? 1 : 0) + s_blobs);
         int kig = 0;
         for (int kb = w.kb0; kb < w.kb1; ++kb) {
@@ -301,9 +332,13 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           if (el) {
             mbar_arrive_expect_tx(full, bytes_data + (has_scales ? bytes_scales : 0));
             if (has_w) bulk_g2s(st, wsrc, kBlobBytes, full);
-            if (n1 > 0) bulk_g2s(st + kPkWBytes, asrc, n1 * kRowBytes, full);
-            if (n2 > 0)   // rows 0.. of the next blob
-              bulk_g2s(st + kPkWBytes + n1 * kRowBytes, asrc + row_pitch - ar0 * kRowBytes, n2 * kRowBytes, full);
+#pragma unroll
+            for (int hh = 0; hh < kHalves; ++hh) {
+              const uint32_t dst = st + kPkWBytes + hh * kPieceRows * kRowBytes;
+              if (n1[hh] > 0) bulk_g2s(dst, asrc[hh], n1[hh] * kRowBytes, full);
+              if (n2[hh] > 0)   // rows 0.. of the next blob
+                bulk_g2s(dst + n1[hh] * kRowBytes, asrc[hh] + row_pitch - ar0[hh] * kRowBytes, n2[hh] * kRowBytes, full);
+            }
             if (has_scales) {
               if (has_w) bulk_g2s(st + kPkWBytes + kPkABytes, swsrc, sc_bytes, full);
               if (s_blobs > 0) bulk_g2s(st + kPkWBytes + kPkABytes + kPkSWBytes, sasrc, sc_bytes, full);
@@ -312,7 +347,8 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
             }
           }
           wsrc += kBlobBytes;
-          asrc += kBlobBytes;
+#pragma unroll
+          for (int hh = 0; hh < kHalves; ++hh) asrc[hh] += kBlobBytes;
           if (kig == 0) { swsrc += sc_bytes / 2; sasrc += sc_bytes / 2; }
           if constexpr (GR::kMultiKb) kig = (kig == kbpg - 1) ? 0 : kig + 1;
           s = (s == kPkStages - 1) ? 0 : s + 1;
@@ -342,23 +378,29 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
 #pragma unroll
           for (int sub = 0; sub < GPK; ++sub) {
             const uint32_t buf = (buf0 + sub) & 1;       // one accumulator buffer per group
-            if (first) {
-              mbar_wait(bar(bAccEmpty + buf), (accpar >> buf) & 1);
-              accpar ^= 1u << buf;
-              tc_fence_after();
-              if (el) stamp(8, kbc);
-            }
 #pragma unroll
-            for (int ks = 0; ks < KS; ++ks) {
-              const int kq = sub * KS + ks;              // K=32 slice of the k-block
-#ifndef APEX4_X_NOMMA   // experiment builds: the barrier protocol without the tensor work
-              if (el) {
-                if (BIAS || ks != 0) mma_i8_ts_pair_lohi<true, kNT>(buf * kNT, a_tm + 8 * kq, blo + 2 * kq, 1u);
-                else mma_i8_ts_pair_lohi<false, kNT>(buf * kNT, a_tm + 8 * kq, blo + 2 * kq, first ? 0u : 1u);
+            for (int hh = 0; hh < kHalves; ++hh) {
+              const uint32_t ab = buf * kHalves + hh;
+              if (first) {
+                mbar_wait(bar(bAccEmpty + ab), (accpar >> ab) & 1);
+                accpar ^= 1u << ab;
+                tc_fence_after();
+                if (el) stamp(8, kbc);
               }
+              const uint32_t d_tm = buf * kNT + hh * T::kMmaN;
+              const uint32_t bh = blo + hh * (kPieceRows * kBlockK >> 4);   // B rows of this half
+#pragma unroll
+              for (int ks = 0; ks < KS; ++ks) {
+                const int kq = sub * KS + ks;            // K=32 slice of the k-block
+#ifndef APEX4_X_NOMMA   // experiment builds: the barrier protocol without the tensor work
+                if (el) {
+                  if (BIAS || ks != 0) mma_i8_ts_pair_lohi<true, T::kMmaN>(d_tm, a_tm + 8 * kq, bh + 2 * kq, 1u);
+                  else mma_i8_ts_pair_lohi<false, T::kMmaN>(d_tm, a_tm + 8 * kq, bh + 2 * kq, first ? 0u : 1u);
+                }
 #endif
+              }
+              if (last && el) tc_commit_pair(bar(bAccFull + ab), 3);
             }
-            if (last && el) tc_commit_pair(bar(bAccFull + buf), 3);
           }
           if (el) tc_commit_pair(bar(bOpEmpty + t), 3);
           if (el) stamp(5, kbc);
@@ -504,6 +546,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
   else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsEpi));
     const int h = (warp - kEpiWarp0) >> 2;              // warpgroup = slice of kEpiCols token columns
+    const int hsel = kHalves == 1 ? 0 : h;              // which full / empty barrier pair of a buffer is ours
     const int lq = warp & 3;                            // TMEM lane quarter this warp may access
     const int epi_tid = threadIdx.x - 32 * kEpiWarp0;
     const uint32_t lane_addr = static_cast<uint32_t>(lq * 32) << 16;
@@ -532,7 +575,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + b), 0);
+      if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + b * kHalves + hsel), 0);
     }
 
     uint32_t gc = 0, item = 0;
@@ -555,33 +598,35 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
       // first TMEM chunk is in flight in v[0].
       constexpr int kVBufs = T::kEpiWGs >= 3 ? 1 : 2;   // three warpgroups hide the TMEM latency by themselves
       uint32_t v[kVBufs][16];
-      uint64_t ab0[2], ab1[2];                           // {a2, b2} of the even / odd group in flight
+      float ab0[2], ab1[2];                              // row scales {a, b} of the even / odd group in flight
       // blocking = false: the barriers were polled earlier (ok != 0: complete)
-      auto group_begin = [&](auto bufc, uint32_t gcx, uint64_t (&ab)[2], bool blocking, uint32_t ok) {
+      auto group_begin = [&](auto bufc, uint32_t gcx, float (&ab)[2], bool blocking, uint32_t ok) {
         constexpr uint32_t BUF = decltype(bufc)::value;
         const int slot = gcx % kScfSlots;
-        if (blocking || !ok) {
-          if (kScfSync) mbar_wait(bar(bScfFull + slot), (gcx / kScfSlots) & 1);
-          mbar_wait(bar(bAccFull + BUF), (fullph >> BUF) & 1);
+        // the polled flag becomes warp-uniform HERE (a vote right behind the poll would expose its latency):
+        // the branch does not diverge, so TMEM addresses stay in uniform registers across it
+        if (blocking || !__all_sync(0xffffffffu, ok)) {
+          if (kScfSync) mbar_wait_warp(bar(bScfFull + slot), (gcx / kScfSlots) & 1);
+          mbar_wait_warp(bar(bAccFull + BUF * kHalves + hsel), (fullph >> BUF) & 1);
         }
         fullph ^= 1u << BUF;
-        float af, bf;
-        unpack_f2(lds64(smem_base + slot * kScfSlotBytes + ab_off), af, bf);
-        ab[0] = pack_f2(af, af);
-        ab[1] = pack_f2(bf, bf);
+        unpack_f2(lds64(smem_base + slot * kScfSlotBytes + ab_off), ab[0], ab[1]);
         tc_fence_after();
 #ifndef APEX4_X_NOLDTM
         tmem_ld_32x16(tm_rd + BUF * kNT, v[0]);
 #endif
       };
-      auto group_body = [&](auto bufc, int gi, const uint64_t (&ab)[2], uint64_t (&ab_next)[2]) {
+      auto group_body = [&](auto bufc, auto morec, int gi, const float (&ab)[2], float (&ab_next)[2]) {
         constexpr uint32_t BUF = decltype(bufc)::value;
+        const bool more = morec;                         // another group of this work item follows (Always: statically)
         const int slot = gc % kScfSlots;
-        const bool more = gi + 1 < ngroups;
         const uint32_t sAf = smem_base + slot * kScfSlotBytes + sa_off;   // + 64 c
         const uint32_t tb = tm_rd + BUF * kNT;
         if (epi_tid == 0) stamp(6, gc);
         uint64_t sq[8];                                  // token scales of the chunk, as pairs
+        // both halves of a packed operand from one register: ptxas uses the broadcast form of FFMA2 (two registers
+        // per group for the row scales instead of four)
+        const uint64_t a2 = pack_f2(ab[0], ab[0]), b2 = pack_f2(ab[1], ab[1]);
         uint32_t ok_next = 0;
 #ifndef APEX4_X_NOEPI   // experiment builds: the epilogue only hands the buffer back
 #pragma unroll
@@ -599,7 +644,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           if (c == (kChunks >= 3 ? kChunks - 3 : 0) && more) {
             // poll the next group's barriers well ahead of their use
             const uint32_t gn = gc + 1;
-            ok_next = mbar_test_wait(bar(bAccFull + (BUF ^ 1)), (fullph >> (BUF ^ 1)) & 1);
+            ok_next = mbar_test_wait(bar(bAccFull + (BUF ^ 1) * kHalves + hsel), (fullph >> (BUF ^ 1)) & 1);
             if (kScfSync) ok_next &= mbar_test_wait(bar(bScfFull + gn % kScfSlots), (gn / kScfSlots) & 1);
           }
 #ifndef APEX4_X_NOLDTM
@@ -607,11 +652,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           if (kVBufs == 2 && c < kChunks - 1) tmem_ld_32x16(tb + 16 * (c + 1), v[(c + 1) % kVBufs]);
 #endif
 #ifndef APEX4_X_NOSTTM
-#ifdef APEX4_X_HYBRID   // timing experiment (wrong results): warpgroup 1 on the I2F path, no re-bias
-          if (BIAS && h == 0) {
-#else
           if constexpr (BIAS) {
-#endif
             tmem_st_32x8(tb + 16 * c, mg);
             tmem_st_32x8(tb + 16 * c + 8, mg);
           }
@@ -620,7 +661,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
             if constexpr (BIAS) tmem_st_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + BUF), 0);
+            if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + BUF * kHalves + hsel), 0);
             if (epi_tid == 0) stamp(16, gc);
             // the next group's first chunk goes into v[0] (chunk kChunks - 2 has been consumed) while the
             // FMAs of this group's last chunk run
@@ -646,20 +687,12 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
 #pragma unroll
           for (int jj = 0; jj < 8; ++jj) {
             uint64_t t0;
-#ifdef APEX4_X_HYBRID
-            if (h == 0) {
-#else
             if constexpr (BIAS) {
-#endif
-#ifdef APEX4_X_FMAINDEP
-              t0 = fma2v(pack_u2(mg[jj & 7], mg[(jj + 1) & 7]), ab[0], ab[1]);
-#else
-              t0 = fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), ab[0], ab[1]);
-#endif
+              t0 = fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2);
             } else {
-              t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[2 * jj])), __int2float_rn(static_cast<int>(vc[2 * jj + 1]))), ab[0]);
+              t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[2 * jj])), __int2float_rn(static_cast<int>(vc[2 * jj + 1]))), a2);
             }
-            acc[c * 8 + jj] = fma2(t0, sq[jj], acc[c * 8 + jj]);   // tokens 16 c + 2 jj, + 1
+            fma2_acc(acc[c * 8 + jj], t0, sq[jj]);   // tokens 16 c + 2 jj, + 1
           }
 #endif
 #ifndef APEX4_X_NOLDTM
@@ -672,7 +705,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
         (void)sq; (void)sAf; (void)tb; (void)ok_next;
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + BUF), 0);
+        if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + BUF * kHalves + hsel), 0);
         if (more) group_begin(std::integral_constant<uint32_t, (BUF ^ 1)>{}, gc + 1, ab_next, true, 0);
 #endif
         if (kScfSync) {
@@ -683,9 +716,28 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
         ++gc;
       };
       if (ngroups > 0) group_begin(std::integral_constant<uint32_t, 0>{}, gc, ab0, true, 0);
-      for (int gi = 0; gi < ngroups; gi += 2) {
-        group_body(std::integral_constant<uint32_t, 0>{}, gi, ab0, ab1);
-        if (gi + 1 < ngroups) group_body(std::integral_constant<uint32_t, 1>{}, gi + 1, ab1, ab0);
+      {
+        // "a group follows" is a compile-time property of each copy of the body: the steady-state pair of
+        // groups is straight-line code (apart from the rare blocking wait), the last one or two are peeled
+        constexpr std::integral_constant<uint32_t, 0> B0{};
+        constexpr std::integral_constant<uint32_t, 1> B1{};
+        int gi = 0;
+        if constexpr (!GR::kMultiKb) {                   // (with groups of several k-blocks the epilogue is off the critical path)
+          for (; gi + 4 < ngroups; gi += 4) {
+            group_body(B0, Always{}, gi, ab0, ab1);
+            group_body(B1, Always{}, gi + 1, ab1, ab0);
+            group_body(B0, Always{}, gi + 2, ab0, ab1);
+            group_body(B1, Always{}, gi + 3, ab1, ab0);
+          }
+          for (; gi + 2 < ngroups; gi += 2) {
+            group_body(B0, Always{}, gi, ab0, ab1);
+            group_body(B1, Always{}, gi + 1, ab1, ab0);
+          }
+        }
+        for (; gi < ngroups; gi += 2) {                  // the last one to four groups: "more" at run time
+          group_body(B0, gi + 1 < ngroups, gi, ab0, ab1);
+          if (gi + 1 < ngroups) group_body(B1, gi + 2 < ngroups, gi + 1, ab1, ab0);
+        }
       }
 
       // ---- a7 (cast + store) or a6 (cross-pair reduce through the FP32 workspace)

@@ -78,6 +78,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   }
 }
 
+// Warp-collective wait: every lane polls, the loop branches on the VOTE of the warp.  A warp-uniform branch
+// keeps the code after it convergent for ptxas -- values in uniform registers (TMEM addresses) stay there, and no
+// BSSY / BSYNC region splits the register allocation of whatever is live across the wait.
+__device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity) {
+  uint32_t spins = 0;
+  while (!__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) {
+    if (++spins > APEX4_WATCHDOG_SPINS) __trap();
+  }
+}
+
 // ------------------------------------------------------------------ bulk async copy (TMA engine, 1-D)
 // global -> shared, completion counted in bytes on an mbarrier.  16-byte aligned, size % 16 == 0.
 __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src_gmem, uint32_t bytes,
@@ -407,6 +417,10 @@ __device__ __forceinline__ uint64_t fma2v(uint64_t a, uint64_t b, uint64_t c) {
   uint64_t d;
   asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
   return d;
+}
+// acc += a * b with the accumulator as ONE read-write operand: the PTX names the same register on both sides
+__device__ __forceinline__ void fma2_acc(uint64_t& acc, uint64_t a, uint64_t b) {
+  asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
 }
 __device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
   uint64_t d;
