@@ -211,6 +211,15 @@ int apex4_measure_rho(double* out_host, void* stream);
  * stream; allocates and frees ~2 KB of device scratch. */
 int apex4_measure_epilogue_pipes(double* out_host, void* stream);
 
+/* The epilogue's own instruction stream in isolation: eight warps per SM take a 192-column accumulator buffer
+ * through registers as the pair kernel's group loop does (tcgen05.ld double-buffered, the tcgen05.st re-bias, token
+ * scales from shared memory, two FMAs per element on 96 accumulators per thread) with no barriers, no MMA, no
+ * wideners.  out_host (HOST, >= 8 doubles): clocks per group for {loads, loads + stores, loads + FMAs,
+ * loads + stores + FMAs, loads + scale loads + FMAs, everything, 0, 0}.  The gap between out[5] and the pair
+ * kernel's measured group period is what the epilogue loses to the warps it shares a sub-partition with and to the
+ * accumulator hand-off.  Synchronises the stream; allocates and frees ~1 KB of device scratch. */
+int apex4_measure_epilogue_stream(double* out_host, void* stream);
+
 /* ---- experiment: is an FP8 tensor-core path exact on INT4 codes? ------------------------------- */
 /* Runs one 128 x 256 tile over K (multiple of 128, <= 32768) through tcgen05.mma kind::i8 and through
  * kind::f8f6f4 with the same codes as E4M3 operands and compares the two TMEM accumulators element by element.

@@ -30,7 +30,7 @@ EXPORTS = (
     "apex4_rmsnorm_quantize", "apex4_silu_mul_quantize",
     "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
     "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes",
-    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_measure_epilogue_pipes",
+    "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_measure_epilogue_pipes", "apex4_measure_epilogue_stream",
     "apex4_e4m3_exactness",
 )
 
@@ -111,6 +111,8 @@ def lib() -> ctypes.CDLL:
     L.apex4_measure_rho.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
     L.apex4_measure_epilogue_pipes.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
     L.apex4_measure_epilogue_pipes.restype = c_int
+    L.apex4_measure_epilogue_stream.argtypes = [ctypes.POINTER(ctypes.c_double), c_void_p]
+    L.apex4_measure_epilogue_stream.restype = c_int
     L.apex4_e4m3_exactness.argtypes = [c_int, c_int, c_int, ctypes.c_uint, ctypes.POINTER(ctypes.c_double), c_void_p]
     L.apex4_e4m3_exactness.restype = c_int
     L.apex4_debug_get_dispatch.argtypes = [c_int] * 6 + [ctypes.POINTER(DebugOpts), ctypes.POINTER(c_int)]
@@ -336,6 +338,14 @@ def measure_epilogue_pipes() -> dict:
     _check(lib().apex4_measure_epilogue_pipes(out, _stream()), "apex4_measure_epilogue_pipes")
     names = {1: "ld", 2: "st", 3: "ld+st", 4: "ffma2", 5: "ld|ffma2", 6: "st|ffma2", 7: "ld+st|ffma2"}
     return {names[m]: {"tmem_clk_per_16_columns": float(out[2 * m]), "ffma2_clk_per_32": float(out[2 * m + 1])} for m in range(1, 8)}
+
+
+def measure_epilogue_stream() -> dict:
+    """apex4_measure_epilogue_stream: clocks per 192-column group of the pair kernel's epilogue stream in isolation."""
+    out = (ctypes.c_double * 8)()
+    _check(lib().apex4_measure_epilogue_stream(out, _stream()), "apex4_measure_epilogue_stream")
+    keys = ("ld", "ld+st", "ld+fma", "ld+st+fma", "ld+lds+fma", "ld+st+lds+fma")
+    return dict(zip(keys, [float(v) for v in out]))
 
 
 def e4m3_exactness(K: int, pattern: int, encoding: int, seed: int = 0) -> dict:

@@ -24,6 +24,7 @@ cudaError_t launch_scales_from_natural(const void* nat, int R, int G, void* tile
 cudaError_t launch_scales_to_natural(const void* tiled, int R, int G, void* nat, cudaStream_t st);
 int measure_rho(double* out, cudaStream_t st);
 int measure_epilogue_pipes(double* out, cudaStream_t st);
+int measure_epilogue_stream(double* out, cudaStream_t st);
 int e4m3_exactness(int K, int pattern, int encoding, uint32_t seed, double* out, cudaStream_t st);
 }  // namespace apex4
 
@@ -461,6 +462,13 @@ int apex4_measure_epilogue_pipes(double* out_host, void* stream) {
   const int a = check_arch();
   if (a != APEX4_OK) return a;
   return measure_epilogue_pipes(out_host, static_cast<cudaStream_t>(stream));
+}
+
+int apex4_measure_epilogue_stream(double* out_host, void* stream) {
+  if (!out_host) return APEX4_ERR_INVALID_ARG;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  return measure_epilogue_stream(out_host, static_cast<cudaStream_t>(stream));
 }
 
 int apex4_measure_rho(double* out_host, void* stream) {

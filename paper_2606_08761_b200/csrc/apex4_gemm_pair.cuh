@@ -52,7 +52,31 @@ namespace apex4 {
 
 namespace pair {
 
+// Biased accumulators (g <= 128).  kind::i8 delivers INT32 sums; turning 96 of them per thread and group into floats
+// with I2F would cost the epilogue as much as its FMAs.  Instead every group's accumulator STARTS at a bias B, so that
+// the word in TMEM, read as binary32, is affine in the group sum P (the operands are 16 q: the sums are 256 P), and the
+// conversion is the FMA that scales anyway: t = fma(word, a, b), acc = fma(t, sA', acc).  Two ways to put the bias there:
+//  * product: B = 0x4B400000 (float 12582912 + 256 P), re-written by the epilogue with tcgen05.st behind every load;
+//    a = sW / 256, b = -49152 sW, sA' = sA;
+//  * -DAPEX4_X_BIASSLICE (tuning build, bit-identical results): the tensor core writes it -- a fifth K = 32 MMA with
+//    accumulate off whose operands are the constant byte 240 read as UNSIGNED 8-bit from 4 KB of shared memory,
+//    32 x 240 x 240 = 1843200 = 256 x 7200 in every element.  256 P lies in [-256 x 7168, 256 x 8192], the word in
+//    [8192, 3940352]: a SUBNORMAL binary32 number of value 2^-149 (1843200 + 256 P); a = sW 2^92, b = -7200 sW 2^-49
+//    (exact), t = P sW 2^-49 rounded once (no underflow: sW >= 2^-24), sA' = sA 2^49.  No tcgen05.st, no constant
+//    registers, the buffer goes back as soon as its last column is in registers -- for 5 tensor-core slices per group
+//    instead of 4.  Measured within 2 % of the product (profiles/r2_gemm_pair_ncu.md): the epilogue is bound by what it
+//    shares the sub-partition with, not by its own instruction stream.
 constexpr uint32_t kMagicBits = 0x4B400000u;   // float 12582912 = 1.5 * 2^23
+#ifdef APEX4_X_BIASSLICE
+constexpr uint32_t kBiasByte = 240;
+constexpr uint32_t kBiasInt = 32u * kBiasByte * kBiasByte;
+constexpr float kBiasP = 7200.0f;
+constexpr int kConstBytes = 4096;              // 128 rows x 32 bytes of the constant
+static_assert(kBiasInt == 256u * 7200u && 7200u >= 7168u && 256u * (7200u + 8192u) < (1u << 23), "bias range");
+#else
+constexpr uint32_t kBiasInt = kMagicBits;
+constexpr int kConstBytes = 0;
+#endif
 #ifndef APEX4_EPI_WGS_192
 #define APEX4_EPI_WGS_192 2          // epilogue warpgroups of the 192-token tile (tuning builds: 3)
 #endif
@@ -121,7 +145,8 @@ struct Tile {
   static constexpr int kScfSlotBytes = kTileRows * 8 + NT * 4 + 256;   // {a,b} per row, sA per column (padded)
   static constexpr int kStoreBytes = kEpiCols * 64;     // per epilogue warp: [kEpiCols m][32 n] FP16 output staging
   static constexpr int kSmemBytes = 1024 + kOpStages * kI8StageBytes + kPkStages * kPkStageBytes +
-                                    kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + kEpiWarps * kStoreBytes;
+                                    kScfSlots * kScfSlotBytes + kNumBars * 8 + 64 + 64 + kEpiWarps * kStoreBytes +
+                                    (kConstBytes ? 128 + kConstBytes : 0);
   static_assert(NT % 64 == 0 && NT <= kPairTokens, "token width");
   static_assert(kAccBufs * NT <= kTmemA0 && kTmemA0 + 32 * kOpStages <= 512, "TMEM columns");
   static_assert(kI8StageBytes % 1024 == 0 && kPkStageBytes % 16 == 0, "alignment");
@@ -264,6 +289,15 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
     fence_mbar_init();
   }
   if (threadIdx.x < 8) reinterpret_cast<volatile uint32_t*>(smem_gen + offMagic)[threadIdx.x] = kMagicBits;
+#ifdef APEX4_X_BIASSLICE
+  constexpr uint32_t offConst = (offStore + kEpiWarps * kStoreBytes + 127) / 128 * 128;   // operands of the bias slice
+  if constexpr (BIAS) {
+    constexpr uint32_t kFill = kBiasByte * 0x01010101u;
+    for (int i = threadIdx.x; i < kConstBytes / 16; i += L::kThreads)
+      reinterpret_cast<uint4*>(smem_gen + offConst)[i] = make_uint4(kFill, kFill, kFill, kFill);
+    fence_proxy_async_smem();     // read by the tcgen05.mma (async proxy) the leader issues, in both CTAs
+  }
+#endif
   if (warp == kCtlWarp0 + 1) tmem_alloc_pair<512>(smem_base + offTmemPtr);
   tc_fence_before();
   __syncthreads();
@@ -361,6 +395,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
     else if (warp == kCtlWarp0 + 1 && rank == 0) {
       const bool el = elect_one();
       const uint32_t desc_lo0 = (((smem_base + offI8) & 0x3FFFFu) >> 4) | (1u << 16);
+#ifdef APEX4_X_BIASSLICE   // the constant operands: any 128 (A) / kHalf (B) rows x 32 bytes inside the 4 KB region
+      const uint64_t cdesc = umma_desc_noswizzle(smem_base + offConst, 128, 256);
+#endif
       uint32_t kbc = 0, t = 0, oppar = 0, accpar = 0;
       while (work_next(p, wit, w, cp, npairs)) {
         int kig = 0;                                     // k-block inside the group (MODE 3)
@@ -389,6 +426,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
               }
               const uint32_t d_tm = buf * kNT + hh * T::kMmaN;
               const uint32_t bh = blo + hh * (kPieceRows * kBlockK >> 4);   // B rows of this half
+#if defined(APEX4_X_BIASSLICE) && !defined(APEX4_X_NOMMA)
+              if (BIAS && el) mma_u8_ss_pair_overwrite<T::kMmaN>(d_tm, cdesc, cdesc);   // the group starts at the bias
+#endif
 #pragma unroll
               for (int ks = 0; ks < KS; ++ks) {
                 const int kq = sub * KS + ks;            // K=32 slice of the k-block
@@ -517,11 +557,16 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
             if (kScfSync) mbar_wait(bar(bScfEmpty + q), ((gc / kScfSlots) & 1) ^ 1);
             float* dstf = reinterpret_cast<float*>(smem_gen + offScf + q * kScfSlotBytes);
             const float sw = __half2float(sWh[sub * kTileRows + r]);
-            const float sa0 = __half2float(sAh[sa_src0 + sub * kTileRows]);
+            float sa0 = __half2float(sAh[sa_src0 + sub * kTileRows]);
             float sa1 = 0.f;
             if (kNT > kTileRows && r + kTileRows < kNT) sa1 = __half2float(sAh[sa_src1 + sub * kTileRows]);
+#ifdef APEX4_X_BIASSLICE
+            reinterpret_cast<float2*>(dstf)[r] = BIAS ? make_float2(sw * 0x1p92f, sw * (-kBiasP * 0x1p-49f)) : make_float2(sw * 0.00390625f, 0.f);
+            if (BIAS) { sa0 *= 0x1p49f; sa1 *= 0x1p49f; }
+#else
             // a = sW / 256 (the operands are 16 q each); b = -12582912 * a removes the magic bias
             reinterpret_cast<float2*>(dstf)[r] = make_float2(sw * 0.00390625f, sw * -49152.0f);
+#endif
             // token scales, in tile order (an epilogue thread reads the 16 of a chunk as four 16-byte vectors)
             if (r < kNT) dstf[2 * kTileRows + r] = sa0;
             if (kNT > kTileRows && r + kTileRows < kNT) dstf[2 * kTileRows + r + kTileRows] = sa1;
@@ -560,19 +605,23 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
     // the magic bias in 8 registers, read through a volatile load so that ptxas keeps them resident
     // instead of re-materialising 16 constants per tcgen05.st (IMAD.MOV on the FMA pipe)
     uint32_t mg[8];
+#ifndef APEX4_X_BIASSLICE
     {
       const uint32_t ma = smem_base + offMagic;
       asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(mg[0]), "=r"(mg[1]), "=r"(mg[2]), "=r"(mg[3]) : "r"(ma));
       asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(mg[4]), "=r"(mg[5]), "=r"(mg[6]), "=r"(mg[7]) : "r"(ma + 16));
     }
+#endif
     // completion #0 of the accEmpty barriers: both buffers start out holding the magic bias
 #pragma unroll
     for (int b = 0; b < kAccBufs; ++b) {
+#ifndef APEX4_X_BIASSLICE
       if (BIAS) {
 #pragma unroll
         for (int c = 0; c < kEpiCols; c += 8) tmem_st_32x8(tmem_base + lane_addr + b * kNT + h * kEpiCols + c, mg);
         tmem_st_wait();
       }
+#endif
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + b * kHalves + hsel), 0);
@@ -651,14 +700,16 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           tmem_ld_wait16(vc);
           if (kVBufs == 2 && c < kChunks - 1) tmem_ld_32x16(tb + 16 * (c + 1), v[(c + 1) % kVBufs]);
 #endif
-#ifndef APEX4_X_NOSTTM
+#if !defined(APEX4_X_NOSTTM) && !defined(APEX4_X_BIASSLICE)
           if constexpr (BIAS) {
             tmem_st_32x8(tb + 16 * c, mg);
             tmem_st_32x8(tb + 16 * c + 8, mg);
           }
 #endif
           if (c == kChunks - 1) {                        // buffer fully read (and re-armed): hand it back
+#ifndef APEX4_X_BIASSLICE
             if constexpr (BIAS) tmem_st_wait();
+#endif
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(bar(bAccEmpty + BUF * kHalves + hsel), 0);
@@ -676,7 +727,7 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
               const int n = n_glob0;
               if (m >= p.pm0 && m < p.pm1 && n >= p.pn0 && n < p.pn1) {
                 const uint32_t x = vc[j];
-                const int32_t raw = static_cast<int32_t>(BIAS ? x - kMagicBits : x);
+                const int32_t raw = static_cast<int32_t>(BIAS ? x - kBiasInt : x);
                 p.P_out[(static_cast<size_t>(m - p.pm0) * (p.pn1 - p.pn0) + (n - p.pn0)) * p.G + gamma] = raw >> 8;
               }
             }
@@ -712,6 +763,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           __syncwarp();
           if (lane == 0) mbar_arrive(bar(bScfEmpty + slot));
         }
+#ifdef APEX4_X_EPIDELAY   // experiment: N idle clocks after every group -- absorbed where the epilogue waits for the MMA warp anyway
+        { const long long t_end = clock64() + APEX4_X_EPIDELAY; while (clock64() < t_end) {} }
+#endif
         if (epi_tid == 0) stamp(7, gc);
         ++gc;
       };

@@ -223,6 +223,11 @@ __host__ __device__ constexpr uint32_t umma_idesc_i8(uint32_t M, uint32_t N) {
   return (2u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 
+// unsigned 8-bit operands (the constant "bias slice" of the pair kernel)
+__host__ __device__ constexpr uint32_t umma_idesc_u8(uint32_t M, uint32_t N) {
+  return (2u << 4) | (0u << 7) | (0u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+}
+
 // ------------------------------------------------------------------ CTA pair (cluster of 2, cta_group::2)
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
@@ -317,6 +322,26 @@ __device__ __forceinline__ void mma_i8_ts_pair_lohi(uint32_t d_tmem, uint32_t a_
         "r"(a_tmem), "r"(b_lo), "n"(kDescHi), "n"(idesc), "r"(accumulate)
         : "memory");
   }
+}
+// D[tmem] = A[smem desc] * B[smem desc]^T (accumulate off), both operands from shared memory, over the CTA pair;
+// descriptors: no swizzle, K-major (LBO between the two 16-byte core-matrix columns of a K = 32 slice, SBO between 8-row groups)
+template <uint32_t N>
+__device__ __forceinline__ void mma_u8_ss_pair_overwrite(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc) {
+  constexpr uint32_t idesc = umma_idesc_u8(256, N);
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, 0, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "n"(idesc)
+      : "memory");
+}
+__device__ __forceinline__ uint64_t umma_desc_noswizzle(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= static_cast<uint64_t>((smem_addr & 0x3FFFFu) >> 4);
+  d |= static_cast<uint64_t>(lbo_bytes >> 4) << 16;
+  d |= static_cast<uint64_t>(sbo_bytes >> 4) << 32;
+  d |= static_cast<uint64_t>(1) << 46;            // version
+  return d;
 }
 __device__ __forceinline__ bool elect_one() {
   uint32_t ok;

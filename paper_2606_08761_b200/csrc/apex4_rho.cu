@@ -192,6 +192,112 @@ int measure_epilogue_pipes(double* out, cudaStream_t st) {
   return cudaGetLastError() == cudaSuccess ? rc : APEX4_ERR_CUDA;
 }
 
+// The epilogue's own instruction stream, in isolation (profiles/r2_gemm_pair_ncu.md): eight warps (two per
+// sub-partition) take a 192-column accumulator buffer through registers exactly as the pair kernel's group loop
+// does -- tcgen05.ld 32x32b.x16 double-buffered, two tcgen05.st 32x32b.x8 of the bias behind each load, the chunk's 16
+// token scales from shared memory, t = fma(word, a, b), acc = fma(t, sA, acc) on 96 accumulators -- with no barriers,
+// no MMA and no wideners.  MODE bit 0 = the re-bias stores, bit 1 = the token-scale loads, bit 2 = the FMAs.
+template <int MODE>
+__global__ void __launch_bounds__(256, 1) epilogue_stream_kernel(int groups, long long* out, float* sink) {
+  __shared__ uint32_t tptr;
+  __shared__ __align__(16) float sa[8][192];
+  const int warp = threadIdx.x >> 5;
+  if (warp == 0) tmem_alloc<512>(smem_u32(&tptr));
+  for (int i = threadIdx.x; i < 8 * 192; i += blockDim.x) (&sa[0][0])[i] = 1.0f + 1e-3f * static_cast<float>(i);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const int h = warp >> 2;
+  const uint32_t tb0 = tptr + (static_cast<uint32_t>((warp & 3) * 32) << 16) + h * 96;
+  uint64_t acc[48];
+#pragma unroll
+  for (int i = 0; i < 48; ++i) acc[i] = 0ull;
+  uint32_t mg[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) mg[i] = 0x4B400000u;
+  asm volatile("" : "+r"(mg[0]), "+r"(mg[1]), "+r"(mg[2]), "+r"(mg[3]), "+r"(mg[4]), "+r"(mg[5]), "+r"(mg[6]), "+r"(mg[7]));
+  for (int b = 0; b < 2; ++b)
+    for (int c = 0; c < 96; c += 8) tmem_st_32x8(tb0 + b * 192 + c, mg);
+  tmem_st_wait();
+  uint32_t v[2][16];
+  float a = 1.0f / 256;
+  const float bb = -49152.0f;
+  const long long t0 = clock64();
+  tmem_ld_32x16(tb0, v[0]);
+  for (int g = 0; g < groups; ++g) {
+    const uint32_t tb = tb0 + (g & 1) * 192;
+    const uint32_t sAf = smem_u32(&sa[g & 7][h * 96]);
+    const uint64_t a2 = pack_f2(a, a), b2 = pack_f2(bb, bb);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      uint32_t* vc = v[c & 1];
+      uint64_t sq[8];
+      if (MODE & 2) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) lds_2x64(sAf + 64 * c + 16 * i, sq[2 * i], sq[2 * i + 1]);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) sq[i] = pack_f2(1.f + i, 2.f + c);
+      }
+      tmem_ld_wait16(vc);
+      tmem_ld_32x16(c < 5 ? tb + 16 * (c + 1) : tb0 + ((g + 1) & 1) * 192, v[(c + 1) & 1]);
+      if (MODE & 1) {
+        tmem_st_32x8(tb + 16 * c, mg);
+        tmem_st_32x8(tb + 16 * c + 8, mg);
+      }
+      if (MODE & 4) {
+#pragma unroll
+        for (int jj = 0; jj < 8; ++jj) fma2_acc(acc[c * 8 + jj], fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2), sq[jj]);
+      } else {
+        acc[c] ^= pack_u2(vc[0] ^ vc[15], vc[8]) ^ sq[0] ^ sq[7];
+      }
+    }
+    a += 1e-6f;
+  }
+  tmem_ld_wait16(v[0]);
+  tmem_st_wait();
+  const long long t1 = clock64();
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < 48; ++i) { float lo, hi; unpack_f2(acc[i], lo, hi); s += lo + hi; }
+  sink[threadIdx.x] = s + __uint_as_float(v[0][0]);
+  if (blockIdx.x == 0 && threadIdx.x == 0) out[0] = t1 - t0;
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) { tc_fence_after(); tmem_dealloc<512>(tptr); }
+}
+
+template <int MODE>
+static double run_epilogue_stream(long long* cyc, float* sink, cudaStream_t st) {
+  const int groups = 2000;
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  for (int rep = 0; rep < 2; ++rep) epilogue_stream_kernel<MODE><<<sms, 256, 0, st>>>(groups, cyc, sink);
+  long long h = 0;
+  if (cudaMemcpyAsync(&h, cyc, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return -1.0;
+  return static_cast<double>(h) / groups;
+}
+
+int measure_epilogue_stream(double* out, cudaStream_t st) {
+  long long* cyc = nullptr;
+  float* sink = nullptr;
+  if (cudaMalloc(&cyc, sizeof(long long)) != cudaSuccess) return APEX4_ERR_CUDA;
+  if (cudaMalloc(&sink, 256 * sizeof(float)) != cudaSuccess) { cudaFree(cyc); return APEX4_ERR_CUDA; }
+  // clocks per 192-column group: loads only; + stores; loads + FMAs; + stores; loads + scales + FMAs; everything
+  out[0] = run_epilogue_stream<0>(cyc, sink, st);
+  out[1] = run_epilogue_stream<1>(cyc, sink, st);
+  out[2] = run_epilogue_stream<4>(cyc, sink, st);
+  out[3] = run_epilogue_stream<5>(cyc, sink, st);
+  out[4] = run_epilogue_stream<6>(cyc, sink, st);
+  out[5] = run_epilogue_stream<7>(cyc, sink, st);
+  out[6] = out[7] = 0.0;
+  cudaFree(cyc);
+  cudaFree(sink);
+  for (int i = 0; i < 6; ++i) if (out[i] < 0.0) return APEX4_ERR_CUDA;
+  return cudaGetLastError() == cudaSuccess ? APEX4_OK : APEX4_ERR_CUDA;
+}
+
 __global__ void clock_probe_kernel(long long* out) {
   unsigned long long g0, g1;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));

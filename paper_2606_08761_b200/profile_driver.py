@@ -6,6 +6,7 @@ number of times on random operands of the right layouts, rotating through operan
     python -m paper_2606_08761_b200.profile_driver time M,N,K,g [...]           sweep-protocol time of the GEMM (one JSON line per shape)
     python -m paper_2606_08761_b200.profile_driver timeline M,N,K,g             device timeline of CTA pair 0 (needs a -DAPEX4_TIMELINE build)
     python -m paper_2606_08761_b200.profile_driver pipes                        apex4_measure_epilogue_pipes table
+    python -m paper_2606_08761_b200.profile_driver stream                       apex4_measure_epilogue_stream table
 
 Variant libraries (the APEX4_X_* / APEX4_TIMELINE tuning switches) are built with
 `python -m paper_2606_08761_b200.build --out /tmp/x.so -DAPEX4_X_NOWIDEN ...` and loaded with APEX4_LIB=/tmp/x.so.
@@ -83,6 +84,10 @@ def main(argv) -> int:
     if len(argv) >= 2 and argv[1] == "pipes":
         for k, v in apex4.measure_epilogue_pipes().items():
             print(f"{k:12s} TMEM warp {v['tmem_clk_per_16_columns']:7.1f} clk / 16 columns   FFMA2 warp {v['ffma2_clk_per_32']:7.1f} clk / 32 FFMA2")
+        return 0
+    if len(argv) >= 2 and argv[1] == "stream":
+        for k, v in apex4.measure_epilogue_stream().items():
+            print(f"{k:16s} {v:7.1f} clk / group (192 columns, 8 warps)")
         return 0
     if len(argv) >= 3 and argv[1] == "time":
         import json

@@ -209,6 +209,16 @@ def test_rho_microbenchmark_ranges(A):
     assert 150 <= r["tmem_ld_bytes_per_clk_sm"] <= 1100, r
 
 
+def test_epilogue_stream_probe_is_ordered(A):
+    """apex4_measure_epilogue_stream: adding work to the stream never makes it faster, the FMA-only stream cannot beat
+    its FMA-pipe time (2 warps x 96 FFMA2 x 2 clk = 384 clk per sub-partition and group), and the full stream stays
+    below the pair kernel's measured group period (~1150 clk)."""
+    r = A.measure_epilogue_stream()
+    assert r["ld"] < r["ld+st"] < r["ld+st+fma"] <= r["ld+st+lds+fma"] * 1.02, r
+    assert r["ld"] < r["ld+fma"] <= r["ld+lds+fma"] * 1.02 and r["ld+lds+fma"] < r["ld+st+lds+fma"], r
+    assert 384 <= r["ld+fma"] <= 700 and 500 <= r["ld+st+lds+fma"] <= 1150, r
+
+
 @pytest.mark.parametrize("encoding", [0, 1])
 def test_e4m3_tensor_path_is_exact_on_int4_codes(A, encoding):
     """SURVEY 8(f)4 experiment (measured fact on B200, recorded in DESIGN.md): tcgen05.mma kind::f8f6f4 with the
