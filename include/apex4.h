@@ -170,6 +170,21 @@ int apex4_w4a4_gemm_ex(const void* qA_packed, const void* sA_f16, const void* qW
                        int gran, int layer, void* workspace, size_t workspace_bytes, void* stream,
                        const apex4_debug_opts* opts);
 
+/* The same GEMM for callers that cannot allocate device memory (CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the stream-K workspace comes from a static __device__ array of
+ * APEX4_STATIC_WORKSPACE_BYTES inside the library (held by every GPU that loads the library until the process
+ * exits) instead of from the caller.  The call allocates and frees nothing; kernels, dispatch and results are those
+ * of apex4_w4a4_gemm (bit-identical).  A problem whose apex4_workspace_bytes() exceeds
+ * APEX4_STATIC_WORKSPACE_BYTES returns APEX4_ERR_WORKSPACE and launches nothing (use apex4_w4a4_gemm with your own
+ * workspace).  All calls share the one array: the bytes a call needs are cleared on `stream` before its launch, and
+ * calls that OVERLAP on the GPU (different streams without a dependency, or concurrent host threads on different
+ * streams) race on it -- serialise them.  Per device: the array's address is resolved on first use with that device
+ * current. */
+#define APEX4_STATIC_WORKSPACE_BYTES (16u << 20)
+int apex4_w4a4_gemm_static_ws(const void* qA_packed, const void* sA_f16, const void* qW_packed,
+                              const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
+                              int gran, int layer, void* stream);
+
 /* End-to-end convenience over the three calls above with HOST activations and HOST output:
  * x_host_f16 [M,K] (HOST, pinned for true asynchrony) -> cudaMemcpyAsync -> apex4_quantize_act ->
  * apex4_w4a4_gemm (weights qW/sW pre-packed on the DEVICE) -> cudaMemcpyAsync -> y_host [M,N] (HOST).

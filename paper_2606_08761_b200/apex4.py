@@ -29,7 +29,8 @@ EXPORTS = (
     "apex4_workspace_bytes_ex", "apex4_status_string", "apex4_quantize_act", "apex4_pack_weights",
     "apex4_rmsnorm_quantize", "apex4_silu_mul_quantize",
     "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
-    "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_linear_host", "apex4_linear_host_scratch_bytes",
+    "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_gemm_static_ws", "apex4_w4a4_linear_host",
+    "apex4_linear_host_scratch_bytes",
     "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_measure_epilogue_pipes", "apex4_measure_epilogue_stream",
     "apex4_e4m3_exactness",
 )
@@ -102,6 +103,9 @@ def lib() -> ctypes.CDLL:
     L.apex4_w4a4_gemm.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int,
                                   c_int, c_int, c_int, c_int, c_void_p, c_size_t, c_void_p]
     L.apex4_w4a4_gemm_ex.argtypes = L.apex4_w4a4_gemm.argtypes + [ctypes.POINTER(DebugOpts)]
+    L.apex4_w4a4_gemm_static_ws.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int,
+                                            c_int, c_int, c_int, c_int, c_void_p]
+    L.apex4_w4a4_gemm_static_ws.restype = c_int
     L.apex4_w4a4_linear_host.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int, c_int,
                                          c_int, c_int, c_int, c_void_p, c_size_t, c_void_p]
     L.apex4_linear_host_scratch_bytes.argtypes = [c_int] * 6
@@ -289,6 +293,23 @@ def w4a4_gemm(qA, sA, qW, sW, M: int, N: int, K: int, group_size=128, gran=GRAN_
         _check(lib().apex4_w4a4_gemm(*args), "apex4_w4a4_gemm")
     else:
         _check(lib().apex4_w4a4_gemm_ex(*args, _opts_ref(opts)), "apex4_w4a4_gemm_ex")
+    return out
+
+
+STATIC_WORKSPACE_BYTES = 16 << 20   # APEX4_STATIC_WORKSPACE_BYTES of include/apex4.h
+
+
+def w4a4_gemm_static_ws(qA, sA, qW, sW, M: int, N: int, K: int, group_size=128, gran=GRAN_GROUP,
+                        layer=LAYER_OTHER, out_dtype=torch.float16, out=None) -> torch.Tensor:
+    """apex4_w4a4_gemm_static_ws: apex4_w4a4_gemm with the stream-K workspace taken from the library's static device
+    array (no allocation inside the call; pass `out` to keep this wrapper allocation-free too).  Problems that need more
+    than STATIC_WORKSPACE_BYTES raise Apex4Error (status APEX4_ERR_WORKSPACE); overlapping calls race on the array."""
+    if out is None:
+        out = torch.empty((M, N), dtype=out_dtype, device=qA.device)
+    code = OUT_F16 if out.dtype == torch.float16 else OUT_F32
+    _check(lib().apex4_w4a4_gemm_static_ws(qA.data_ptr(), sA.data_ptr(), qW.data_ptr(), sW.data_ptr(), out.data_ptr(),
+                                           code, M, N, K, group_size, gran, layer, _stream()),
+           "apex4_w4a4_gemm_static_ws")
     return out
 
 

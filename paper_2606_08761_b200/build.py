@@ -13,7 +13,8 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libapex4.so")
-SOURCES = ["apex4_api.cu", "apex4_quant.cu", "apex4_fused_quant.cu", "apex4_gemm_pair.cu", "apex4_gemm_pair_m0.cu", "apex4_gemm_pair_m1.cu", "apex4_gemm_pair_m2.cu", "apex4_gemm_pair_m3.cu", "apex4_gemv.cu", "apex4_rho.cu", "apex4_e4m3.cu"]
+SOURCES = ["apex4_api.cu", "apex4_quant.cu", "apex4_fused_quant.cu", "apex4_gemm_pair.cu", "apex4_gemm_pair_m0.cu", "apex4_gemm_pair_m1.cu", "apex4_gemm_pair_m2.cu", "apex4_gemm_pair_m3.cu", "apex4_gemv.cu", "apex4_rho.cu", "apex4_e4m3.cu",
+           "apex4_static_ws.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
     "-Xcompiler", "-fPIC", "--shared",
