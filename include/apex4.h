@@ -107,8 +107,9 @@ size_t apex4_packed_bytes(int R, int K);
 size_t apex4_scale_elems(int R, int K, int g);
 /* Bytes of DEVICE workspace apex4_w4a4_gemm needs for this problem.  0 when every output tile is
  * computed by one CTA (pair) alone: the decode kernels (M <= 32 at g <= 128 or per-channel) and any tile count that
- * fills the SMs evenly.  Otherwise (stream-K, a6) it holds the tile arrival counters followed by the
- * FP32 partial sums of the shared tiles (padded to whole tiles).  The workspace must be zero-filled
+ * fills the SMs evenly.  Otherwise (stream-K, a6) it holds, per CTA pair of the launch, two arrival counters and
+ * one 256 x tile-width FP32 tile for the output tile that pair shares with its successors: at most ~14.6 MB on a
+ * B200 (74 pairs x 256 x 192 x 4 B), independent of M and N.  The workspace must be zero-filled
  * once by the caller before its first use; every call leaves it zero-filled again, so one buffer
  * serves any sequence of calls on one stream.  Concurrent calls on different streams need their own. */
 size_t apex4_workspace_bytes(int M, int N, int K, int group_size, int gran, int layer);
@@ -176,7 +177,8 @@ int apex4_w4a4_gemm_ex(const void* qA_packed, const void* sA_f16, const void* qW
  * exits) instead of from the caller.  The call allocates and frees nothing; kernels, dispatch and results are those
  * of apex4_w4a4_gemm (bit-identical).  A problem whose apex4_workspace_bytes() exceeds
  * APEX4_STATIC_WORKSPACE_BYTES returns APEX4_ERR_WORKSPACE and launches nothing (use apex4_w4a4_gemm with your own
- * workspace).  All calls share the one array: the bytes a call needs are cleared on `stream` before its launch, and
+ * workspace); with one workspace slot per CTA pair that cannot happen on a 148-SM B200 (<= 14.6 MB), it is the
+ * guard for devices with more SMs.  All calls share the one array: the bytes a call needs are cleared on `stream` before its launch, and
  * calls that OVERLAP on the GPU (different streams without a dependency, or concurrent host threads on different
  * streams) race on it -- serialise them.  Per device: the array's address is resolved on first use with that device
  * current. */

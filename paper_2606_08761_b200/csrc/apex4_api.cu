@@ -157,8 +157,10 @@ bool choose_dispatch(int M, int N, int K, int g, const apex4_debug_opts& o, Disp
   return true;
 }
 
+// Stream-K workspace: one slot per CTA pair (a shared tile's slot is the pair that owns its first unit, see the
+// kernel), each an arrival counter per CTA and a 256 x pnt FP32 tile -- independent of M and N.
 size_t counters_bytes(const Dispatch& d) {
-  return (static_cast<size_t>(d.tiles_m) * d.tiles_n * 2 * 4 + 255) / 256 * 256;
+  return (static_cast<size_t>(d.grid) * 2 * 4 + 255) / 256 * 256;
 }
 
 cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, cudaStream_t st) {
@@ -169,8 +171,8 @@ cudaError_t launch_dispatch(const GemmParams& p, const Dispatch& d, bool dump, c
 }
 size_t workspace_need(const Dispatch& d) {
   if (!d.split) return 0;
-  // every 256 x pnt pair tile as FP32 in fragment order (tile-padded), after the arrival counters
-  return counters_bytes(d) + static_cast<size_t>(d.tiles_m) * d.tiles_n * 256 * d.pnt * 4;
+  // per slot a 256 x pnt pair tile as FP32 in fragment order, after the arrival counters
+  return counters_bytes(d) + static_cast<size_t>(d.grid) * 256 * d.pnt * 4;
 }
 
 int validate_gemm_shape(int M, int N, int K) {

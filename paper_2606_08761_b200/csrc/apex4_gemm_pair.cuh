@@ -842,12 +842,17 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           store_tile();
         } else {
           // a6: FP32 partial sums meet in the workspace ("inter-SM global reduction").  The
-          // workspace holds every CTA tile in FRAGMENT order -- [tile][CTA][j][thread][4 floats] --
+          // workspace holds one CTA tile per SLOT in FRAGMENT order -- [slot][CTA][j][thread][4 floats] --
           // so a partial tile is fully coalesced red.global.add.v4.f32 per thread (not scalar atomics),
           // and the CTA that completes the tile reads it back with the same thread mapping,
           // leaves it zero-filled, casts and stores.
-          float* wst = p.ws + static_cast<size_t>((w.nt * p.tiles_m + w.mt) * 2 + static_cast<int>(rank)) * (kTileRows * kNT) +
-                       epi_tid * 4;
+          // Slot of a shared tile = the pair whose unit range holds the tile's FIRST unit.  Ranges are contiguous, so
+          // two shared tiles never have the same first-unit owner (the earlier one would lie wholly inside that
+          // pair's range and not be shared): npairs slots suffice, whatever M and N are.
+          const long long first_unit = static_cast<long long>(w.nt * p.tiles_m + w.mt) * p.upt;
+          const long long total_units = static_cast<long long>(p.tiles_m) * p.tiles_n * p.upt;
+          const int slot = static_cast<int>(((first_unit + 1) * static_cast<int>(gridDim.x >> 1) - 1) / total_units);
+          float* wst = p.ws + static_cast<size_t>(slot * 2 + static_cast<int>(rank)) * (kTileRows * kNT) + epi_tid * 4;
 #pragma unroll
           for (int j = 0; j < 4 * kChunks; ++j) {
             float f0, f1, f2, f3;
@@ -862,11 +867,11 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           int* flag = reinterpret_cast<int*>(smem_gen + offTmemPtr + 8);
           asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
           if (epi_tid == 0) {
-            const int tile = (w.nt * p.tiles_m + w.mt) * 2 + static_cast<int>(rank);
-            const int prev = atomicAdd(p.counters + tile, w.units);
+            const int cslot = slot * 2 + static_cast<int>(rank);
+            const int prev = atomicAdd(p.counters + cslot, w.units);
             const int done = (prev + w.units == p.upt);
             *flag = done;
-            if (done) p.counters[tile] = 0;
+            if (done) p.counters[cslot] = 0;
           }
           asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
           const int done = *flag;

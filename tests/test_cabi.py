@@ -84,11 +84,12 @@ def test_dispatch_table(L):
     assert (kern, width, split, upt) == (DEC, 16, 0, 7) and 1 <= grid <= 148
     assert apex4.debug_get_dispatch(32, 8192, 8192, 128)[:2] == (DEC, 32)
     assert apex4.workspace_bytes(16, 8192, 8192, 128) == 0
-    # 32 < M <= 64: CTA pairs on 256 x 64 tiles, 32 tiles on <= 74 pairs -> stream-K; workspace = 32 * 2
-    # counters + every 256 x 64 tile as FP32
+    # 32 < M <= 64: CTA pairs on 256 x 64 tiles, 32 tiles on <= 74 pairs -> stream-K; the workspace has one slot per
+    # CTA pair (2 arrival counters, padded to 256 bytes in total, + a 256 x 64 FP32 tile), whatever M and N are
     kern, width, split, grid, upt = apex4.debug_get_dispatch(64, 8192, 8192, 128)
     assert (kern, width, split, upt) == (PAIR, 64, 1, 64)
-    assert apex4.workspace_bytes(64, 8192, 8192, 128) == 256 + 32 * 256 * 64 * 4
+    pad256 = lambda n: (n + 255) // 256 * 256
+    assert apex4.workspace_bytes(64, 8192, 8192, 128) == pad256(grid * 8) + grid * 256 * 64 * 4
     # M = 256: two 128-token tiles instead of a 192-token tile and a third-full one
     assert apex4.debug_get_dispatch(256, 4096, 4096, 128)[1] == 128
     # tensor-bound regime: CTA pairs on 256 x 192 tiles; 43 x 32 tiles fill the last wave -> whole tiles
@@ -98,8 +99,10 @@ def test_dispatch_table(L):
     # Llama-2-7B O-proj at M = 2048: 11 x 16 tiles on <= 74 pairs -> stream-K with the FP32 workspace
     kern, width, split, grid, upt = apex4.debug_get_dispatch(2048, 4096, 4096, 128)
     assert (kern, width, split, upt) == (PAIR, 192, 1, 32)
-    # 11 * 16 * 2 counters (padded to 256 bytes) + every 256 x 192 tile as FP32 in fragment order
-    assert apex4.workspace_bytes(2048, 4096, 4096, 128) == 1536 + 11 * 16 * 256 * 192 * 4
+    # per CTA pair: 2 counters + a 256 x 192 tile as FP32 in fragment order -- at most ~14.6 MB on 74 pairs
+    assert apex4.workspace_bytes(2048, 4096, 4096, 128) == pad256(grid * 8) + grid * 256 * 192 * 4
+    assert apex4.workspace_bytes(2048, 4096, 4096, 128) <= 16 << 20
+    assert apex4.workspace_bytes(4096, 57344, 8192, 32) <= 16 << 20
     # per-channel decode: the streaming kernel with an exact INT32 cross-warp reduction, no workspace
     assert apex4.debug_get_dispatch(16, 8192, 8192, 0, apex4.GRAN_CHANNEL)[:3] == (DEC, 16, 0)
     assert apex4.workspace_bytes(16, 8192, 8192, 8192) == 0
@@ -114,7 +117,7 @@ def test_dispatch_table(L):
     # per-call options: forcing the pair kernel / a tile width / stream-K changes this call only
     o = apex4.debug_opts(kernel=PAIR, pair_tokens=128, split=1, grid=5)
     assert apex4.debug_get_dispatch(16, 256, 512, 128, opts=o)[:4] == (PAIR, 128, 1, 4)   # 4 units: grid capped
-    assert apex4.workspace_bytes(16, 256, 512, 128, opts=o) == 256 + 256 * 128 * 4
+    assert apex4.workspace_bytes(16, 256, 512, 128, opts=o) == 256 + 4 * 256 * 128 * 4           # one slot per pair of the launch
     assert apex4.debug_get_dispatch(16, 256, 512, 128)[0] == DEC                           # ... not the next one
     with pytest.raises(apex4.Apex4Error):            # the decode kernel does not cover M > 32
         apex4.debug_get_dispatch(64, 256, 512, 128, opts=apex4.debug_opts(kernel=DEC))
