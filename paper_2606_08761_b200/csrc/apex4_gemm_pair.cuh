@@ -741,7 +741,11 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
             if constexpr (BIAS) {
               t0 = fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2);
             } else {
+#ifdef APEX4_X_IADDMAGIC   // tuning build: unbiased accumulators, the magic bias added in registers (one integer add per element)
+              t0 = fma2v(pack_u2(vc[2 * jj] + kMagicBits, vc[2 * jj + 1] + kMagicBits), a2, b2);
+#else
               t0 = mul2(pack_f2(__int2float_rn(static_cast<int>(vc[2 * jj])), __int2float_rn(static_cast<int>(vc[2 * jj + 1]))), a2);
+#endif
             }
             fma2_acc(acc[c * 8 + jj], t0, sq[jj]);   // tokens 16 c + 2 jj, + 1
           }
