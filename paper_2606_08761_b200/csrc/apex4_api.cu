@@ -85,13 +85,15 @@ const apex4_debug_opts kAuto = {-1, 0, -1, 0, 0, nullptr};
 // a 192-token tile per token (measured at N = K = 8192, g = 128: M = 1024 110.1 vs 111.5 us, M = 512 60.3 vs 65.4 us,
 // M = 256 32.6 vs 41.6 us, M = 4096 the 192-token tile).  M <= 64: the 64-token tile; up to 128 tokens it also wins
 // while all its tiles still fit one wave (M = 128, N = 8192: 24.6 us against 26.0 us on one 128-token tile row).
-int pair_tokens(int M, int N, const apex4_debug_opts& o) {
+// Groups of several k-blocks (g > 128) are tensor-bound, not epilogue-bound: there a 128-token tile costs ~1.2 x a
+// 192-token tile per token (M = 1024 per-channel: 78.2 vs 71.6 us), so it is taken only when it saves more than that.
+int pair_tokens(int M, int N, int g, const apex4_debug_opts& o) {
   if (o.pair_tokens > 0) return o.pair_tokens;
   if (M <= 64) return 64;
   const int tiles_n = (N + 2 * kTileRows - 1) / (2 * kTileRows);
   if (M <= 128 && 2 * tiles_n <= gemm_max_pairs()) return 64;
   const int r128 = (M + 127) / 128 * 128, r192 = (M + kPairTokens - 1) / kPairTokens * kPairTokens;
-  return 11 * r128 < 10 * r192 ? 128 : kPairTokens;
+  return (g > kBlockK ? 6 * r128 < 5 * r192 : 11 * r128 < 10 * r192) ? 128 : kPairTokens;
 }
 
 // The decode kernel covers M <= 32 at g = 32 / 64 / 128, per-channel, and the group sizes in between whose
@@ -137,7 +139,7 @@ bool choose_dispatch(int M, int N, int K, int g, const apex4_debug_opts& o, Disp
     if (o.decode_batch > 0 && o.decode_batch < d.upt) d.upt = o.decode_batch;
     return true;
   }
-  d.pnt = pair_tokens(M, N, o);
+  d.pnt = pair_tokens(M, N, g, o);
   if (d.pnt != 64 && d.pnt != 128 && d.pnt != kPairTokens) return false;
   d.tiles_m = (M + d.pnt - 1) / d.pnt;
   d.tiles_n = (N + 2 * kTileRows - 1) / (2 * kTileRows);
