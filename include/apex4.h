@@ -171,6 +171,23 @@ int apex4_w4a4_gemm_ex(const void* qA_packed, const void* sA_f16, const void* qW
                        int gran, int layer, void* workspace, size_t workspace_bytes, void* stream,
                        const apex4_debug_opts* opts);
 
+/* ---- K-split (row-parallel) tensor parallelism, the reduce-scatter fused into the GEMM ------ */
+/* This rank holds the K-slice [k0, k1) of X and W (cut on group boundaries: qA/sA from apex4_quantize_act on the
+ * slice, qW/sW packed from the slice, K_local = k1 - k0).  Output column n belongs to rank n / (N / world);
+ * owner_y_f32[r] (a HOST array of `world` DEVICE pointers) is rank r's FP32 accumulation buffer [M, N / world]
+ * row-major -- this rank's own memory for r == rank, peer memory mapped over NVLink (CUDA IPC / cudaMemcpyPeer-
+ * capable mapping, P2P access enabled) for the others.  The epilogue of the GEMM kernels ADDS each finished
+ * FP32 partial tile into its owner's buffer with red.global.add.f32 (system scope) as the tiles complete, so the
+ * exchange overlaps the math tile by tile: one kernel is GEMM + reduce-scatter; no Y is stored.
+ * Protocol (the caller's, e.g. paper_2606_08761_b200/tp.py): every rank zero-fills its own buffer; barrier; every
+ * rank calls this; barrier (after stream completion); each rank reads / casts its [M, N / world] slice.
+ * N % world == 0, (N / world) % 8 == 0, world <= 8; workspace as for apex4_w4a4_gemm at (M, N, K_local).
+ * Per-group integer sums are those of the single-GPU path; only the FP32 summation order over ranks (and
+ * tiles, atomics) varies -- inside the output tolerance (R12), not bitwise reproducible. */
+int apex4_w4a4_gemm_tp_push(const void* qA_packed, const void* sA_f16, const void* qW_packed, const void* sW_f16,
+                            void* const* owner_y_f32, int world, int M, int N, int K_local, int group_size, int gran,
+                            int layer, void* workspace, size_t workspace_bytes, void* stream);
+
 /* The same GEMM for callers that cannot allocate device memory (CUDA graph capture, tight serving loops,
  * harnesses that forbid cudaMalloc): the stream-K workspace comes from a static __device__ array of
  * APEX4_STATIC_WORKSPACE_BYTES inside the library (held by every GPU that loads the library until the process

@@ -29,7 +29,7 @@ EXPORTS = (
     "apex4_workspace_bytes_ex", "apex4_status_string", "apex4_quantize_act", "apex4_pack_weights",
     "apex4_rmsnorm_quantize", "apex4_silu_mul_quantize",
     "apex4_pack_codes", "apex4_scales_from_natural", "apex4_scales_to_natural", "apex4_unpack_codes",
-    "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_gemm_static_ws", "apex4_w4a4_linear_host",
+    "apex4_w4a4_gemm", "apex4_w4a4_gemm_ex", "apex4_w4a4_gemm_static_ws", "apex4_w4a4_gemm_tp_push", "apex4_w4a4_linear_host",
     "apex4_linear_host_scratch_bytes",
     "apex4_debug_group_sums", "apex4_debug_get_dispatch", "apex4_measure_rho", "apex4_measure_epilogue_pipes", "apex4_measure_epilogue_stream",
     "apex4_e4m3_exactness",
@@ -106,6 +106,9 @@ def lib() -> ctypes.CDLL:
     L.apex4_w4a4_gemm_static_ws.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int,
                                             c_int, c_int, c_int, c_int, c_void_p]
     L.apex4_w4a4_gemm_static_ws.restype = c_int
+    L.apex4_w4a4_gemm_tp_push.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, ctypes.POINTER(c_void_p), c_int, c_int, c_int,
+                                          c_int, c_int, c_int, c_int, c_void_p, c_size_t, c_void_p]
+    L.apex4_w4a4_gemm_tp_push.restype = c_int
     L.apex4_w4a4_linear_host.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int, c_int,
                                          c_int, c_int, c_int, c_void_p, c_size_t, c_void_p]
     L.apex4_linear_host_scratch_bytes.argtypes = [c_int] * 6
@@ -294,6 +297,20 @@ def w4a4_gemm(qA, sA, qW, sW, M: int, N: int, K: int, group_size=128, gran=GRAN_
     else:
         _check(lib().apex4_w4a4_gemm_ex(*args, _opts_ref(opts)), "apex4_w4a4_gemm_ex")
     return out
+
+
+def w4a4_gemm_tp_push(qA, sA, qW, sW, owner_ptrs, M: int, N: int, K_local: int, group_size=128, gran=GRAN_GROUP,
+                      layer=LAYER_OTHER, workspace=None) -> None:
+    """apex4_w4a4_gemm_tp_push: this rank's K-slice GEMM whose epilogue adds the FP32 partial tiles into the owners'
+    [M, N / world] buffers (owner_ptrs: device addresses, one per rank; peers' buffers mapped over NVLink)."""
+    world = len(owner_ptrs)
+    arr = (ctypes.c_void_p * world)(*[int(v) if v else None for v in owner_ptrs])
+    if workspace is None:
+        workspace = make_workspace(M, N, K_local, group_size, gran, layer, qA.device)
+    wp = workspace.data_ptr() if workspace is not None else None
+    wb = workspace.numel() if workspace is not None else 0
+    _check(lib().apex4_w4a4_gemm_tp_push(qA.data_ptr(), sA.data_ptr(), qW.data_ptr(), sW.data_ptr(), arr, world, M, N, K_local,
+                                         group_size, gran, layer, wp, wb, _stream()), "apex4_w4a4_gemm_tp_push")
 
 
 STATIC_WORKSPACE_BYTES = 16 << 20   # APEX4_STATIC_WORKSPACE_BYTES of include/apex4.h

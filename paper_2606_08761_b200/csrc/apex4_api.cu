@@ -365,6 +365,38 @@ int apex4_w4a4_gemm_ex(const void* qA_packed, const void* sA_f16, const void* qW
              : APEX4_ERR_CUDA;
 }
 
+int apex4_w4a4_gemm_tp_push(const void* qA_packed, const void* sA_f16, const void* qW_packed, const void* sW_f16,
+                            void* const* owner_y_f32, int world, int M, int N, int K_local, int group_size, int gran,
+                            int layer, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!qA_packed || !sA_f16 || !qW_packed || !sW_f16 || !owner_y_f32) return APEX4_ERR_INVALID_ARG;
+  if (world < 1 || world > kMaxPushRanks) return APEX4_ERR_INVALID_ARG;
+  int v = validate_gemm_shape(M, N, K_local);
+  if (v != APEX4_OK) return v;
+  if (N % world != 0 || (N / world) % 8 != 0) return APEX4_ERR_UNSUPPORTED_SHAPE;   // whole 8-column pieces per owner
+  const int g = resolve_g(K_local, group_size, gran, layer);
+  if (g < 0) return -g;
+  if (!aligned16(qA_packed) || !aligned16(sA_f16) || !aligned16(qW_packed) || !aligned16(sW_f16)) return APEX4_ERR_ALIGNMENT;
+  for (int r = 0; r < world; ++r)
+    if (!owner_y_f32[r] || !aligned16(owner_y_f32[r])) return owner_y_f32[r] ? APEX4_ERR_ALIGNMENT : APEX4_ERR_INVALID_ARG;
+  const int a = check_arch();
+  if (a != APEX4_OK) return a;
+  Dispatch d;
+  if (!choose_dispatch(M, N, K_local, g, kAuto, d)) return APEX4_ERR_INVALID_ARG;
+  GemmParams p;
+  fill_params(p, d, qA_packed, sA_f16, qW_packed, sW_f16, M, N, K_local, g);
+  p.Y = owner_y_f32[0];   // non-null: "there is an output"; the push path never stores through it
+  p.out_f32 = 1;
+  p.push = 1;
+  p.push_cols = N / world;
+  for (int r = 0; r < world; ++r) p.push_y[r] = static_cast<float*>(owner_y_f32[r]);
+  if (d.split) {
+    if (!workspace || workspace_bytes < workspace_need(d) || !aligned16(workspace)) return APEX4_ERR_WORKSPACE;
+    p.counters = static_cast<int*>(workspace);
+    p.ws = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + counters_bytes(d));
+  }
+  return launch_dispatch(p, d, false, static_cast<cudaStream_t>(stream)) == cudaSuccess ? APEX4_OK : APEX4_ERR_CUDA;
+}
+
 int apex4_w4a4_gemm(const void* qA_packed, const void* sA_f16, const void* qW_packed,
                     const void* sW_f16, void* Y, int out_dtype, int M, int N, int K, int group_size,
                     int gran, int layer, void* workspace, size_t workspace_bytes, void* stream) {

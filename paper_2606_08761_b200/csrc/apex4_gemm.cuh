@@ -29,7 +29,13 @@ struct GemmParams {
   int32_t* P_out;      // debug dump of the per-group INT32 sums (DUMP kernels only)
   int pm0, pm1, pn0, pn1;
   long long* tl;       // -DAPEX4_TIMELINE builds only: clock64 stamps of CTA 0, [event][64]; else unused
+  // Tensor-parallel K-split (apex4_w4a4_gemm_tp_push): instead of storing Y the epilogue ADDS its FP32 partial tile
+  // into the owner's accumulation buffer -- output column n belongs to rank n / push_cols, whose buffer
+  // push_y[rank] is [M, push_cols] FP32 row-major and may be peer memory mapped over NVLink (red.global.add.f32).
+  int push, push_cols;
+  float* push_y[8];
 };
+constexpr int kMaxPushRanks = 8;
 
 // Launch with programmatic stream serialization (PDL): the kernel may start while its predecessor on the
 // stream drains; it calls griddep_wait() (apex4_ptx.cuh) before it touches anything the predecessor wrote.

@@ -233,7 +233,7 @@ __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Wor
 
 using namespace pair;
 
-template <int MODE, bool DUMP, int NT>
+template <int MODE, bool DUMP, int NT, bool PUSH = false>
 __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenWGs, Tile<NT>::kEpiWGs>::kLaunchRegs))
     w4a4_gemm_pair_kernel(const GemmParams p) {
   using GR = Gran<MODE>;
@@ -832,6 +832,21 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
           }
           float* y = static_cast<float*>(p.Y);      // FP32 output: lanes = consecutive n, coalesced rows
           if (n_glob0 < p.N) {
+            if constexpr (PUSH) {   // (its own instantiation: the product kernel's code is untouched)
+              // K-split tensor parallelism: the partial tile is added into the buffer of the rank that owns these
+              // columns (possibly over NVLink), tile by tile as the GEMM proceeds -- GEMM and reduce-scatter in one kernel
+              const int owner = n_glob0 / p.push_cols;
+              float* yo = p.push_y[owner] + (n_glob0 - owner * p.push_cols);
+#pragma unroll
+              for (int x = 0; x < 8 * kChunks; ++x) {
+                float f0, f1;
+                unpack_f2(acc[x], f0, f1);
+                const int m = m_glob0 + 2 * x;
+                if (m < p.M) asm volatile("red.relaxed.sys.global.add.f32 [%0], %1;" ::"l"(yo + static_cast<size_t>(m) * p.push_cols), "f"(f0) : "memory");
+                if (m + 1 < p.M) asm volatile("red.relaxed.sys.global.add.f32 [%0], %1;" ::"l"(yo + static_cast<size_t>(m + 1) * p.push_cols), "f"(f1) : "memory");
+              }
+              return;
+            }
 #pragma unroll
             for (int x = 0; x < 8 * kChunks; ++x) {
               float f0, f1;
@@ -910,9 +925,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
 }
 
 // ------------------------------------------------------------------------------------ launcher
-template <int MODE, bool DUMP, int NT>
+template <int MODE, bool DUMP, int NT, bool PUSH = false>
 static cudaError_t launch_pair_one(const GemmParams& p, int npairs, cudaStream_t st) {
-  auto kern = w4a4_gemm_pair_kernel<MODE, DUMP, NT>;
+  auto kern = w4a4_gemm_pair_kernel<MODE, DUMP, NT, PUSH>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<NT>::kSmemBytes);
   if (e != cudaSuccess) return e;
   kern<<<2 * npairs, Warps<Gran<MODE>::kWidenWGs, Tile<NT>::kEpiWGs>::kThreads, Tile<NT>::kSmemBytes, st>>>(p);
@@ -926,6 +941,14 @@ cudaError_t launch_pair_mode(const GemmParams& p, bool dump, int npairs, cudaStr
 #define APEX4_PAIR_INSTANTIATE(MODE)                                                                     \
   template <>                                                                                            \
   cudaError_t launch_pair_mode<MODE>(const GemmParams& p, bool dump, int npairs, cudaStream_t st) {      \
+    if (p.push && !dump) {                                                                               \
+      switch (p.pair_nt) {                                                                               \
+        case 64: return launch_pair_one<MODE, false, 64, true>(p, npairs, st);                           \
+        case 128: return launch_pair_one<MODE, false, 128, true>(p, npairs, st);                         \
+        case kPairTokens: return launch_pair_one<MODE, false, kPairTokens, true>(p, npairs, st);         \
+        default: return cudaErrorInvalidValue;                                                           \
+      }                                                                                                  \
+    }                                                                                                    \
     switch (p.pair_nt) {                                                                                 \
       case 64: return dump ? launch_pair_one<MODE, true, 64>(p, npairs, st) : launch_pair_one<MODE, false, 64>(p, npairs, st);   \
       case 128: return dump ? launch_pair_one<MODE, true, 128>(p, npairs, st) : launch_pair_one<MODE, false, 128>(p, npairs, st); \

@@ -458,7 +458,12 @@ __global__ void __launch_bounds__(kThreads, 1) w4a4_gemv_kernel(const GemmParams
           }
           }
           if (p.Y != nullptr && n < p.N) {
-            if (p.out_f32) {
+            if (p.push) {     // K-split tensor parallelism: add into the owner rank's FP32 buffer (see GemmParams)
+              const int owner = n / p.push_cols;
+              float* yo = p.push_y[owner] + (n - owner * p.push_cols);
+              if (m < p.M) asm volatile("red.relaxed.sys.global.add.v2.f32 [%0], {%1, %2};" ::"l"(yo + static_cast<size_t>(m) * p.push_cols), "f"(v.x), "f"(v.y) : "memory");
+              if (m + 8 < p.M) asm volatile("red.relaxed.sys.global.add.v2.f32 [%0], {%1, %2};" ::"l"(yo + static_cast<size_t>(m + 8) * p.push_cols), "f"(v.z), "f"(v.w) : "memory");
+            } else if (p.out_f32) {
               float* y = static_cast<float*>(p.Y);
               if (m < p.M) *reinterpret_cast<float2*>(y + static_cast<size_t>(m) * p.N + n) = make_float2(v.x, v.y);
               if (m + 8 < p.M) *reinterpret_cast<float2*>(y + static_cast<size_t>(m + 8) * p.N + n) = make_float2(v.z, v.w);

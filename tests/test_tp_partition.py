@@ -28,6 +28,18 @@ def test_k_split_properties():
         k_split(4000, 32, 2)
 
 
+def test_owner_columns_of_the_fused_reduce_scatter():
+    from paper_2606_08761_b200.tp import owner_columns
+    for N, world in [(8192, 8), (4096, 2), (384, 3), (1024, 1), (57344, 7)]:
+        cols = owner_columns(N, world)
+        assert len(cols) == world and cols[0][0] == 0 and cols[-1][1] == N
+        assert all(b - a == N // world and a % 8 == 0 for a, b in cols)
+        assert all(cols[i][1] == cols[i + 1][0] for i in range(world - 1))
+    for N, world in [(4096, 3), (8200, 4), (24, 2)]:        # unequal pieces / pieces that are not whole 8-column units
+        with pytest.raises(ValueError):
+            owner_columns(N, world)
+
+
 WORKER = r"""
 import os, sys
 import numpy as np, torch, torch.distributed as dist
