@@ -130,6 +130,15 @@ inline int gran_mode(int g) { return g == kBlockK ? 0 : g == 64 ? 1 : g == 32 ? 
 
 // Everything that depends on the token width NT of the pair tile (MMA N = accumulator buffer width):
 // 192 in the tensor-bound regime, 128 / 64 where M would leave most of a 192-token tile empty.
+// Widener warpgroups for (MODE, NT): two where the wideners, not the epilogue, set the pace -- groups of several
+// k-blocks (MODE 3), and (tuning switch APEX4_X_WWG_NT: token width up to which two are used) narrow token tiles, whose
+// epilogue is short while a k-block's 128 weight rows cost the wideners the same ~750 clk whatever the token width is.
+#ifndef APEX4_X_WWG_NT
+#define APEX4_X_WWG_NT 0
+#endif
+template <int MODE, int NT>
+__host__ __device__ constexpr int widen_wgs() { return (Gran<MODE>::kWidenWGs == 2 || NT <= APEX4_X_WWG_NT) ? 2 : Gran<MODE>::kWidenWGs; }
+
 template <int NT>
 struct Tile {
   static constexpr int kNT = NT;
@@ -234,10 +243,10 @@ __device__ __forceinline__ bool work_next(const GemmParams& p, WorkIter& it, Wor
 using namespace pair;
 
 template <int MODE, bool DUMP, int NT, bool PUSH = false>
-__global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenWGs, Tile<NT>::kEpiWGs>::kLaunchRegs))
+__global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<widen_wgs<MODE, NT>(), Tile<NT>::kEpiWGs>::kLaunchRegs))
     w4a4_gemm_pair_kernel(const GemmParams p) {
   using GR = Gran<MODE>;
-  using L = Warps<GR::kWidenWGs, Tile<NT>::kEpiWGs>;
+  using L = Warps<widen_wgs<MODE, NT>(), Tile<NT>::kEpiWGs>;
   using T = Tile<NT>;
   constexpr bool BIAS = GR::kBias;
   constexpr int GPK = GR::kGpk;
@@ -255,6 +264,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
   uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   asm volatile("" : "+r"(smem_base));
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+#ifdef APEX4_TIMELINE   // event 18: kernel entry / set-up done / before / after the teardown barrier (thread 0 of CTA 0, 1)
+  if (p.tl != nullptr && blockIdx.x < 2 && threadIdx.x == 0) p.tl[(blockIdx.x * 32 + 18) * 64 + 0] = clock64();
+#endif
 
   constexpr uint32_t offI8 = 0;
   constexpr uint32_t offPk = offI8 + kOpStages * kI8StageBytes;
@@ -306,6 +318,9 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + offTmemPtr);
   if (tmem_base != 0) __trap();   // the whole TMEM (512 columns) is ours: lane 0, column 0
 
+#ifdef APEX4_TIMELINE
+  if (p.tl != nullptr && blockIdx.x < 2 && threadIdx.x == 0) p.tl[(blockIdx.x * 32 + 18) * 64 + 1] = clock64();
+#endif
   WorkIter wit;
   Work w;
   work_begin(p, wit, cp, npairs);
@@ -917,7 +932,13 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<Gran<MODE>::kWidenW
 
   // ---- teardown: nobody leaves while the peer may still signal this CTA's barriers or read its
   // shared memory / TMEM through the pair MMA
+#ifdef APEX4_TIMELINE
+  if (p.tl != nullptr && blockIdx.x < 2 && (threadIdx.x & 31) == 0) p.tl[(blockIdx.x * 32 + 19) * 64 + (threadIdx.x >> 5)] = clock64();   // per warp: done
+#endif
   cluster_sync_all();
+#ifdef APEX4_TIMELINE
+  if (p.tl != nullptr && blockIdx.x < 2 && threadIdx.x == 0) p.tl[(blockIdx.x * 32 + 18) * 64 + 3] = clock64();
+#endif
   if (warp == kCtlWarp0 + 1) {
     tc_fence_after();
     tmem_dealloc_pair<512>(tmem_base);
@@ -930,7 +951,7 @@ static cudaError_t launch_pair_one(const GemmParams& p, int npairs, cudaStream_t
   auto kern = w4a4_gemm_pair_kernel<MODE, DUMP, NT, PUSH>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<NT>::kSmemBytes);
   if (e != cudaSuccess) return e;
-  kern<<<2 * npairs, Warps<Gran<MODE>::kWidenWGs, Tile<NT>::kEpiWGs>::kThreads, Tile<NT>::kSmemBytes, st>>>(p);
+  kern<<<2 * npairs, Warps<widen_wgs<MODE, NT>(), Tile<NT>::kEpiWGs>::kThreads, Tile<NT>::kSmemBytes, st>>>(p);
   return cudaGetLastError();
 }
 
