@@ -317,6 +317,13 @@ __global__ void __cluster_dims__(2, 1, 1) __maxnreg__((Warps<widen_wgs<MODE, NT>
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + offTmemPtr);
   if (tmem_base != 0) __trap();   // the whole TMEM (512 columns) is ours: lane 0, column 0
+#ifndef APEX4_X_NOPDL
+  // Programmatic dependent launch: the set-up above (barriers, TMEM, cluster rendezvous) overlapped the tail of the
+  // predecessor on the stream (the online quantizer); from here on its output is complete and visible.  The successor
+  // may be scheduled as soon as SMs free up; every kernel of this library waits before it reads or writes global memory.
+  griddep_launch();
+  griddep_wait();
+#endif
 
 #ifdef APEX4_TIMELINE
   if (p.tl != nullptr && blockIdx.x < 2 && threadIdx.x == 0) p.tl[(blockIdx.x * 32 + 18) * 64 + 1] = clock64();
@@ -951,8 +958,13 @@ static cudaError_t launch_pair_one(const GemmParams& p, int npairs, cudaStream_t
   auto kern = w4a4_gemm_pair_kernel<MODE, DUMP, NT, PUSH>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile<NT>::kSmemBytes);
   if (e != cudaSuccess) return e;
+#ifdef APEX4_X_NOPDL
   kern<<<2 * npairs, Warps<widen_wgs<MODE, NT>(), Tile<NT>::kEpiWGs>::kThreads, Tile<NT>::kSmemBytes, st>>>(p);
   return cudaGetLastError();
+#else
+  e = launch_pdl(kern, dim3(2 * npairs), dim3(Warps<widen_wgs<MODE, NT>(), Tile<NT>::kEpiWGs>::kThreads), Tile<NT>::kSmemBytes, st, p);
+  return e != cudaSuccess ? e : cudaGetLastError();
+#endif
 }
 
 // defined (explicitly instantiated) in apex4_gemm_pair_m<MODE>.cu
