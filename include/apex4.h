@@ -249,7 +249,8 @@ int apex4_measure_epilogue_pipes(double* out_host, void* stream);
  * through registers as the pair kernel's group loop does (tcgen05.ld double-buffered, the tcgen05.st re-bias, token
  * scales from shared memory, two FMAs per element on 96 accumulators per thread) with no barriers, no MMA, no
  * wideners.  out_host (HOST, >= 8 doubles): clocks per group for {loads, loads + stores, loads + FMAs,
- * loads + stores + FMAs, loads + scale loads + FMAs, everything, 0, 0}.  The gap between out[5] and the pair
+ * loads + stores + FMAs, loads + scale loads + FMAs, everything, and -- for the alternative tcgen05.ld.16x256b fragment
+ * layout (four rows x four tokens per thread and chunk: a quarter of the token-scale loads) -- loads, everything}.  The gap between out[5] and the pair
  * kernel's measured group period is what the epilogue loses to the warps it shares a sub-partition with and to the
  * accumulator hand-off.  Synchronises the stream; allocates and frees ~1 KB of device scratch. */
 int apex4_measure_epilogue_stream(double* out_host, void* stream);

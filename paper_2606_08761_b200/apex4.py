@@ -382,7 +382,7 @@ def measure_epilogue_stream() -> dict:
     """apex4_measure_epilogue_stream: clocks per 192-column group of the pair kernel's epilogue stream in isolation."""
     out = (ctypes.c_double * 8)()
     _check(lib().apex4_measure_epilogue_stream(out, _stream()), "apex4_measure_epilogue_stream")
-    keys = ("ld", "ld+st", "ld+fma", "ld+st+fma", "ld+lds+fma", "ld+st+lds+fma")
+    keys = ("ld", "ld+st", "ld+fma", "ld+st+fma", "ld+lds+fma", "ld+st+lds+fma", "16x256b: ld", "16x256b: ld+st+lds+fma")
     return dict(zip(keys, [float(v) for v in out]))
 
 

@@ -197,11 +197,22 @@ int measure_epilogue_pipes(double* out, cudaStream_t st) {
 // does -- tcgen05.ld 32x32b.x16 double-buffered, two tcgen05.st 32x32b.x8 of the bias behind each load, the chunk's 16
 // token scales from shared memory, t = fma(word, a, b), acc = fma(t, sA, acc) on 96 accumulators -- with no barriers,
 // no MMA and no wideners.  MODE bit 0 = the re-bias stores, bit 1 = the token-scale loads, bit 2 = the FMAs.
-template <int MODE>
+// LAYOUT 1 is the alternative fragment layout that was considered for the kernel: two tcgen05.ld.16x256b.x2 per 16-column
+// chunk give a thread four weight rows x four tokens instead of one row x sixteen, so it needs one 16-byte load of token
+// scales per chunk instead of four (and four {a, b} row pairs per group instead of one).
+__device__ __forceinline__ void tmem_ld_16x256_x2(uint32_t taddr, uint32_t* v) {
+  asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
+}
+template <int MODE, int LAYOUT = 0>
 __global__ void __launch_bounds__(256, 1) epilogue_stream_kernel(int groups, long long* out, float* sink) {
   __shared__ uint32_t tptr;
   __shared__ __align__(16) float sa[8][192];
-  const int warp = threadIdx.x >> 5;
+  __shared__ __align__(8) float rowab[128][2];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x < 128) { rowab[threadIdx.x][0] = 1.0f / 256; rowab[threadIdx.x][1] = -49152.0f; }
   if (warp == 0) tmem_alloc<512>(smem_u32(&tptr));
   for (int i = threadIdx.x; i < 8 * 192; i += blockDim.x) (&sa[0][0])[i] = 1.0f + 1e-3f * static_cast<float>(i);
   tc_fence_before();
@@ -222,32 +233,58 @@ __global__ void __launch_bounds__(256, 1) epilogue_stream_kernel(int groups, lon
   uint32_t v[2][16];
   float a = 1.0f / 256;
   const float bb = -49152.0f;
+  auto load_chunk = [&](uint32_t addr, uint32_t (&d)[16]) {
+    if constexpr (LAYOUT == 0) {
+      tmem_ld_32x16(addr, d);
+    } else {
+      tmem_ld_16x256_x2(addr, d);                       // lanes 0-15 of the warp's quarter
+      tmem_ld_16x256_x2(addr + (16u << 16), d + 8);     // lanes 16-31
+    }
+  };
   const long long t0 = clock64();
-  tmem_ld_32x16(tb0, v[0]);
+  load_chunk(tb0, v[0]);
   for (int g = 0; g < groups; ++g) {
     const uint32_t tb = tb0 + (g & 1) * 192;
     const uint32_t sAf = smem_u32(&sa[g & 7][h * 96]);
     const uint64_t a2 = pack_f2(a, a), b2 = pack_f2(bb, bb);
+    float ra[4], rb[4];                                 // LAYOUT 1: {a, b} of the thread's four rows
+    if constexpr (LAYOUT == 1) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) unpack_f2(lds64(smem_u32(&rowab[(warp & 3) * 32 + (lane >> 2) + 8 * i][0])), ra[i], rb[i]);
+    }
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       uint32_t* vc = v[c & 1];
       uint64_t sq[8];
       if (MODE & 2) {
+        if constexpr (LAYOUT == 0) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) lds_2x64(sAf + 64 * c + 16 * i, sq[2 * i], sq[2 * i + 1]);
+          for (int i = 0; i < 4; ++i) lds_2x64(sAf + 64 * c + 16 * i, sq[2 * i], sq[2 * i + 1]);
+        } else {
+          lds_2x64(sAf + 64 * c + 16 * (lane & 3), sq[0], sq[1]);   // the thread's four columns of the chunk (slot permuted)
+        }
       } else {
 #pragma unroll
         for (int i = 0; i < 8; ++i) sq[i] = pack_f2(1.f + i, 2.f + c);
       }
       tmem_ld_wait16(vc);
-      tmem_ld_32x16(c < 5 ? tb + 16 * (c + 1) : tb0 + ((g + 1) & 1) * 192, v[(c + 1) & 1]);
+      load_chunk(c < 5 ? tb + 16 * (c + 1) : tb0 + ((g + 1) & 1) * 192, v[(c + 1) & 1]);
       if (MODE & 1) {
         tmem_st_32x8(tb + 16 * c, mg);
         tmem_st_32x8(tb + 16 * c + 8, mg);
       }
       if (MODE & 4) {
+        if constexpr (LAYOUT == 0) {
 #pragma unroll
-        for (int jj = 0; jj < 8; ++jj) fma2_acc(acc[c * 8 + jj], fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2), sq[jj]);
+          for (int jj = 0; jj < 8; ++jj) fma2_acc(acc[c * 8 + jj], fma2v(pack_u2(vc[2 * jj], vc[2 * jj + 1]), a2, b2), sq[jj]);
+        } else {
+          // registers of one load: {row 0 pair 0, row 1 pair 0, row 0 pair 1, row 1 pair 1}; the second load: rows 2, 3
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const int row = 2 * (q >> 2) + (q & 1), pr = (q >> 1) & 1;
+            fma2_acc(acc[c * 8 + q], fma2v(pack_u2(vc[2 * q], vc[2 * q + 1]), pack_f2(ra[row], ra[row]), pack_f2(rb[row], rb[row])), sq[pr]);
+          }
+        }
       } else {
         acc[c] ^= pack_u2(vc[0] ^ vc[15], vc[8]) ^ sq[0] ^ sq[7];
       }
@@ -267,13 +304,13 @@ __global__ void __launch_bounds__(256, 1) epilogue_stream_kernel(int groups, lon
   if (warp == 0) { tc_fence_after(); tmem_dealloc<512>(tptr); }
 }
 
-template <int MODE>
+template <int MODE, int LAYOUT = 0>
 static double run_epilogue_stream(long long* cyc, float* sink, cudaStream_t st) {
   const int groups = 2000;
   int dev = 0, sms = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  for (int rep = 0; rep < 2; ++rep) epilogue_stream_kernel<MODE><<<sms, 256, 0, st>>>(groups, cyc, sink);
+  for (int rep = 0; rep < 2; ++rep) epilogue_stream_kernel<MODE, LAYOUT><<<sms, 256, 0, st>>>(groups, cyc, sink);
   long long h = 0;
   if (cudaMemcpyAsync(&h, cyc, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return -1.0;
   return static_cast<double>(h) / groups;
@@ -291,10 +328,12 @@ int measure_epilogue_stream(double* out, cudaStream_t st) {
   out[3] = run_epilogue_stream<5>(cyc, sink, st);
   out[4] = run_epilogue_stream<6>(cyc, sink, st);
   out[5] = run_epilogue_stream<7>(cyc, sink, st);
-  out[6] = out[7] = 0.0;
+  // the 16x256b fragment layout: loads only; everything
+  out[6] = run_epilogue_stream<0, 1>(cyc, sink, st);
+  out[7] = run_epilogue_stream<7, 1>(cyc, sink, st);
   cudaFree(cyc);
   cudaFree(sink);
-  for (int i = 0; i < 6; ++i) if (out[i] < 0.0) return APEX4_ERR_CUDA;
+  for (int i = 0; i < 8; ++i) if (out[i] < 0.0) return APEX4_ERR_CUDA;
   return cudaGetLastError() == cudaSuccess ? APEX4_OK : APEX4_ERR_CUDA;
 }
 

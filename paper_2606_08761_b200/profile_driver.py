@@ -87,7 +87,7 @@ def main(argv) -> int:
         return 0
     if len(argv) >= 2 and argv[1] == "stream":
         for k, v in apex4.measure_epilogue_stream().items():
-            print(f"{k:16s} {v:7.1f} clk / group (192 columns, 8 warps)")
+            print(f"{k:24s} {v:7.1f} clk / group (192 columns, 8 warps)")
         return 0
     if len(argv) >= 3 and argv[1] == "time":
         import json
